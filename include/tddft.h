@@ -1,0 +1,149 @@
+/* tddft.h -- C ABI of the B200-native TDA Liouville (Casida-A) operator of plane-wave hybrid LR-TDDFT
+ * (arXiv 2309.03513, "WEST-TDDFT"), Gamma point, real orbitals.
+ *
+ * The library applies   A = D + K1e - K1d   (Eq. 9; terms: Eq. 3, Eq. 4
+ * PAPER.md:82-85, Eq. 6) and its spin-flip counterpart  D^SF - K1d^SF  (PAPER.md:162-182,
+ * Eqs. 21, 23, 25) to a block of trial vectors, and finds the lowest roots with a block Davidson solver
+ * (PAPER.md:274).  Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions:
+ *   lattice rows a_i (bohr), Omega = |det A|, reciprocal rows b_i with b_i.a_j = 2 pi delta_ij,
+ *   G = m1 b1 + m2 b2 + m3 b3, grid point r_j = sum_i (j_i/n_i) a_i.
+ *   Wavefunction sphere |G|^2 <= ecut_wfc_ry (|G|^2 in bohr^-2 equals the kinetic energy in Ry).
+ *   Real orbitals: c(-G) = conj c(G); only the canonical HALF sphere is stored: npwh complex coefficients,
+ *   G = 0 first with Im c(0) = 0.  phi(r) = Omega^-1/2 sum_G c(G) exp(i G.r), sum_G |c(G)|^2 = 1.
+ *   Inner product of half-sphere vectors: <a|b> = 2 Re sum_half conj(a) b - a(0) b(0).
+ *   Energies in Hartree, cutoff in Ry.
+ *
+ * Trial-vector layout (Eq. 2: one function per occupied orbital and spin):
+ *   one vector = [spin block][v][g], complex128 interleaved, contiguous; a block of nvec vectors is [k][...].
+ *   spin conserving: blocks = spins 0..nspin-1, block s has nocc[s] functions; length = sum_s nocc[s] * npwh
+ *   spin flip (up -> down):   one block of nocc[0] functions (occupied-up index v, living in the down space)
+ *   spin flip (down -> up):   one block of nocc[1] functions
+ *
+ * Ownership: the caller owns every buffer.  psi_up/psi_dn (and vloc_*) are BORROWED for the life of the
+ * context and must stay valid and unchanged.  The library allocates its own device workspace in tddft_init.
+ * Unless stated otherwise pointers named "device" are CUDA device pointers and "host" are host pointers.
+ *
+ * Errors: every call returns a tddft_status; nothing throws or aborts across the ABI.  CUDA failures give
+ * TDDFT_ECUDA with the text available from tddft_last_error.  A context is not thread-safe.
+ * All device work is issued on the stream given in tddft_options (default: the legacy default stream).
+ * tddft_apply_liouville is asynchronous with respect to the host; tddft_davidson and the *_host variant
+ * synchronise the stream before returning.
+ */
+#ifndef TDDFT_H
+#define TDDFT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tddft_ctx tddft_ctx; /* opaque; one per problem */
+
+typedef enum {
+  TDDFT_SPIN_CONSERVING = 0,   /* Eq. 9 */
+  TDDFT_SPIN_FLIP = 1,         /* Eq. 21, up occupied -> down virtual: sigma~ = up, sigma = down */
+  TDDFT_SPIN_FLIP_DOWN_UP = 2  /* Eq. 21, down occupied -> up virtual */
+} tddft_mode;
+
+typedef enum {
+  TDDFT_OK = 0,
+  TDDFT_EINVAL = 1,        /* bad argument (message in tddft_last_error) */
+  TDDFT_ENOMEM = 2,        /* host or device allocation failed */
+  TDDFT_ECUDA = 3,         /* a CUDA call or kernel failed */
+  TDDFT_ENOTCONVERGED = 4, /* Davidson hit max_iter; outputs hold the best estimates */
+  TDDFT_EUNSUPPORTED = 5   /* valid request this build cannot serve (e.g. an FFT length without a plan) */
+} tddft_status;
+
+/* All fields optional: pass NULL for defaults, or zero-initialise and set struct_size = sizeof(tddft_options). */
+typedef struct {
+  int struct_size;          /* ABI versioning: sizeof(tddft_options) of the caller */
+  int use_hartree_fxc;      /* spin-conserving K1e (Eq. 4): 1 = on (default), 0 = off; set -1 for "default" */
+  double rho_floor;         /* f_xc = 0 where a spin density is below this; <= 0 means default 1e-10 */
+  const double* vloc_up;    /* device, [n1*n2*n3] real, optional local potential of the model H (reading A4) */
+  const double* vloc_dn;    /* device, idem for spin down (ignored when nspin = 1) */
+  void* cuda_stream;        /* cudaStream_t; NULL = legacy default stream */
+  double workspace_gb;      /* cap on the library's device workspace; <= 0 = 85 % of free memory at init */
+  int pair_tile;            /* orbitals per tile edge T of the exchange loop; <= 0 = chosen from the workspace */
+  int fft_batch;            /* packed pair grids per FFT launch; <= 0 = default */
+  /* Davidson (reading A11) */
+  int max_subspace;         /* <= 0: 12 * nroots */
+  int max_iter;             /* <= 0: 200 */
+  double tol;               /* residual 2-norm; <= 0: 1e-6 */
+  const double* x0;         /* device, n_x0 start vectors in the mode's layout, or NULL: library draws its own */
+  int n_x0;
+  unsigned long long seed;  /* seed of the library's own start vectors */
+} tddft_options;
+
+/* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,
+ * or m1=0,m2>0, or m1=m2=0,m3>0; ordered by ascending |G|^2 (1e-12 relative ties) then (m1,m2,m3).
+ * lattice: host, 9 doubles row-major (rows a1,a2,a3, bohr).  miller: host int[3*capacity] or NULL to query.
+ * g2: host double[capacity] or NULL (|G|^2 in bohr^-2).  *npwh receives the count.
+ * Returns TDDFT_EINVAL if capacity is too small (count still reported).  Callable before tddft_init. */
+int tddft_enumerate_gvectors(const double* lattice, double ecut_wfc_ry, long capacity, int* miller, double* g2,
+                             long* npwh);
+
+/* Build a context: G sphere and index maps, Coulomb table 4 pi/|G|^2 (G=0 zeroed),
+ * phi_vs(r) for all occupied orbitals, rho0_s = sum_v phi^2 and the LDA f_xc (Eq. 8).
+ *   grid:  host int[3], each length must have an FFT plan (2-3-5 smooth, <= 256) and hold the sphere
+ *   nspin: 1 (closed shell, singlet channel, reading A6; psi_dn/eig_dn ignored) or 2
+ *   nocc:  host int[2]
+ *   psi_*: DEVICE complex128 [nocc][npwh], canonical G order, orthonormal (not checked)
+ *   eig_*: HOST double[nocc], Hartree
+ *   alpha: fraction of exact exchange, >= 0 */
+int tddft_init(tddft_ctx** ctx, const double* lattice, const int* grid, double ecut_wfc_ry, int nspin,
+               const int* nocc, const double* psi_up, const double* psi_dn, const double* eig_up,
+               const double* eig_dn, double alpha, const tddft_options* opt);
+
+int tddft_npw_half(const tddft_ctx* ctx, long* npwh);
+/* miller: host int[3*npwh] in canonical order */
+int tddft_gvectors(const tddft_ctx* ctx, int* miller);
+/* complex elements of one trial vector in the given mode */
+int tddft_vector_len(const tddft_ctx* ctx, int mode, long* n_complex);
+/* bytes of device workspace the context holds */
+int tddft_workspace_bytes(const tddft_ctx* ctx, long long* bytes);
+
+/* AX = A X for a block of nvec trial vectors.  X, AX: DEVICE complex128 [nvec][vector_len],
+ * X read-only, AX must not alias X.  The operator projects its output only (Eqs. 3-6 apply P_c on the left). */
+int tddft_apply_liouville(tddft_ctx* ctx, const double* X, double* AX, int nvec, int mode);
+
+/* Same with HOST buffers: copies X to the device, applies, copies AX back, synchronises. */
+int tddft_apply_liouville_host(tddft_ctx* ctx, const double* X_host, double* AX_host, int nvec, int mode);
+
+/* Lowest nroots of A by block Davidson (reading A11).
+ *   evals:    HOST double[nroots], ascending, Hartree
+ *   evecs:    DEVICE complex128 [nroots][vector_len] or NULL
+ *   iters:    HOST int* or NULL, iterations used
+ *   resnorms: HOST double[nroots] or NULL, final residual 2-norms */
+int tddft_davidson(tddft_ctx* ctx, int nroots, int mode, double* evals, double* evecs, int* iters,
+                   double* resnorms);
+
+/* Counters of the last tddft_apply_liouville call (for benchmarks): kernels launched, unique pair potentials
+ * tau_vv' formed, and the milliseconds each stage took if timing was enabled. */
+typedef struct {
+  long long kernel_launches;
+  long long pair_ffts;
+  double ms_total, ms_s1_to_real, ms_s23_hxc, ms_s4_pair_fft, ms_s5_contract, ms_s6_to_sphere, ms_s8_project;
+} tddft_stats;
+int tddft_set_timing(tddft_ctx* ctx, int enabled); /* stage timing with CUDA events (adds synchronisation) */
+int tddft_get_stats(const tddft_ctx* ctx, tddft_stats* out);
+
+/* Stand-alone pieces of the hot path, exposed for unit parity tests and micro-benchmarks.
+ * tddft_pair_potentials: tau_p = C[phi_i phi_j] for n_pairs orbital pairs of one spin;
+ *   pairs: HOST int[2*n_pairs]; tau: DEVICE double [n_pairs][n1*n2*n3].
+ * tddft_project: Y <- P_c Y on nfun half-sphere functions of target spin `spin`;
+ *   Y: DEVICE complex128 [nfun][npwh], in place.
+ * tddft_gram: G[i][j] = <V_i|W_j> for m x m full trial vectors; V, W DEVICE [m][n_complex], G HOST. */
+int tddft_pair_potentials(tddft_ctx* ctx, int spin, const int* pairs, long n_pairs, double* tau);
+int tddft_project(tddft_ctx* ctx, int spin, double* Y, long nfun);
+int tddft_gram(tddft_ctx* ctx, const double* V, const double* W, int m, long n_complex, double* G);
+/* real-space orbital phi_v of a spin on the FFT grid, DEVICE double [n1*n2*n3] out */
+int tddft_orbital_real_space(tddft_ctx* ctx, int spin, int v, double* out);
+
+const char* tddft_last_error(const tddft_ctx* ctx); /* ctx may be NULL: error of the last failed tddft_init */
+int tddft_destroy(tddft_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDDFT_H */

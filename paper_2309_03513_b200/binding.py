@@ -1,0 +1,219 @@
+"""Thin ctypes binding of libtddft_b200.so: argument marshalling only, same names as include/tddft.h.
+
+Every numerical step runs inside the CUDA library.  PyTorch supplies device memory and streams only.
+Importing this module never falls back to a CPU implementation: if the shared library is missing the
+import raises, and if no CUDA device is present `tddft_init` returns TDDFT_ECUDA.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtddft_b200.so")
+
+TDDFT_SPIN_CONSERVING, TDDFT_SPIN_FLIP, TDDFT_SPIN_FLIP_DOWN_UP = 0, 1, 2
+TDDFT_OK, TDDFT_EINVAL, TDDFT_ENOMEM, TDDFT_ECUDA, TDDFT_ENOTCONVERGED, TDDFT_EUNSUPPORTED = range(6)
+
+EXPORTS = [
+    "tddft_enumerate_gvectors", "tddft_init", "tddft_npw_half", "tddft_gvectors", "tddft_vector_len",
+    "tddft_workspace_bytes", "tddft_apply_liouville", "tddft_apply_liouville_host", "tddft_davidson",
+    "tddft_set_timing", "tddft_get_stats", "tddft_pair_potentials", "tddft_project", "tddft_gram",
+    "tddft_orbital_real_space", "tddft_last_error", "tddft_destroy",
+]
+
+
+class tddft_options(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_int), ("use_hartree_fxc", C.c_int), ("rho_floor", C.c_double),
+        ("vloc_up", C.c_void_p), ("vloc_dn", C.c_void_p), ("cuda_stream", C.c_void_p),
+        ("workspace_gb", C.c_double), ("pair_tile", C.c_int), ("fft_batch", C.c_int),
+        ("max_subspace", C.c_int), ("max_iter", C.c_int), ("tol", C.c_double),
+        ("x0", C.c_void_p), ("n_x0", C.c_int), ("seed", C.c_ulonglong),
+    ]
+
+
+class tddft_stats(C.Structure):
+    _fields_ = [("kernel_launches", C.c_longlong), ("pair_ffts", C.c_longlong), ("ms_total", C.c_double),
+                ("ms_s1_to_real", C.c_double), ("ms_s23_hxc", C.c_double), ("ms_s4_pair_fft", C.c_double),
+                ("ms_s5_contract", C.c_double), ("ms_s6_to_sphere", C.c_double), ("ms_s8_project", C.c_double)]
+
+
+def load_library():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libtddft_b200.so is not built: run `python -m paper_2309_03513_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.tddft_last_error.restype = C.c_char_p
+    lib.tddft_last_error.argtypes = [C.c_void_p]
+    return lib
+
+
+_lib = load_library()
+
+
+class TddftError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("tddft status %d: %s" % (status, msg))
+        self.status = status
+
+
+def _check(rc, ctx=None):
+    if rc != TDDFT_OK:
+        msg = _lib.tddft_last_error(ctx)
+        raise TddftError(rc, msg.decode() if msg else "")
+
+
+def _ptr(t):
+    """Device (torch tensor) or raw integer pointer."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    return C.c_void_p(t.data_ptr())
+
+
+def tddft_enumerate_gvectors(lattice, ecut_wfc_ry):
+    """Returns (miller[npwh,3] int32, g2[npwh] float64)."""
+    lat = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
+    n = C.c_long(0)
+    rc = _lib.tddft_enumerate_gvectors(lat.ctypes.data_as(C.c_void_p), C.c_double(ecut_wfc_ry), C.c_long(0), None, None, C.byref(n))
+    _check(rc)
+    miller = np.zeros((n.value, 3), dtype=np.int32)
+    g2 = np.zeros(n.value, dtype=np.float64)
+    rc = _lib.tddft_enumerate_gvectors(lat.ctypes.data_as(C.c_void_p), C.c_double(ecut_wfc_ry), C.c_long(n.value),
+                                       miller.ctypes.data_as(C.c_void_p), g2.ctypes.data_as(C.c_void_p), C.byref(n))
+    _check(rc)
+    return miller, g2
+
+
+class Context:
+    """Owns a tddft_ctx*.  Keeps references to the borrowed device tensors (psi, vloc, x0) alive."""
+
+    def __init__(self, handle, keep):
+        self._h = handle
+        self._keep = keep
+
+    def destroy(self):
+        if self._h:
+            _lib.tddft_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def tddft_init(lattice, grid, ecut_wfc_ry, nspin, nocc, psi_up, psi_dn, eig_up, eig_dn, alpha, **opt):
+    """psi_*: CUDA torch tensors complex128 [nocc, npwh]; eig_*: host arrays; opt: fields of tddft_options."""
+    lat = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
+    g = (C.c_int * 3)(*[int(x) for x in grid])
+    no = (C.c_int * 2)(int(nocc[0]), int(nocc[1]) if len(nocc) > 1 else 0)
+    eu = np.ascontiguousarray(eig_up, dtype=np.float64)
+    ed = None if eig_dn is None else np.ascontiguousarray(eig_dn, dtype=np.float64)
+    o = tddft_options()
+    o.struct_size = C.sizeof(tddft_options)
+    o.use_hartree_fxc = -1
+    keep = [psi_up, psi_dn]
+    for k, v in opt.items():
+        if k in ("vloc_up", "vloc_dn", "x0"):
+            keep.append(v)
+            setattr(o, k, None if v is None else v.data_ptr())
+        elif k == "cuda_stream":
+            o.cuda_stream = v
+        else:
+            setattr(o, k, v)
+    h = C.c_void_p(None)
+    rc = _lib.tddft_init(C.byref(h), lat.ctypes.data_as(C.c_void_p), g, C.c_double(ecut_wfc_ry), C.c_int(nspin), no,
+                         _ptr(psi_up), _ptr(psi_dn), eu.ctypes.data_as(C.c_void_p),
+                         None if ed is None else ed.ctypes.data_as(C.c_void_p), C.c_double(alpha), C.byref(o))
+    _check(rc)
+    return Context(h, keep)
+
+
+def tddft_npw_half(ctx):
+    n = C.c_long(0)
+    _check(_lib.tddft_npw_half(ctx._h, C.byref(n)), ctx._h)
+    return n.value
+
+
+def tddft_gvectors(ctx):
+    m = np.zeros((tddft_npw_half(ctx), 3), dtype=np.int32)
+    _check(_lib.tddft_gvectors(ctx._h, m.ctypes.data_as(C.c_void_p)), ctx._h)
+    return m
+
+
+def tddft_vector_len(ctx, mode):
+    n = C.c_long(0)
+    _check(_lib.tddft_vector_len(ctx._h, C.c_int(mode), C.byref(n)), ctx._h)
+    return n.value
+
+
+def tddft_workspace_bytes(ctx):
+    n = C.c_longlong(0)
+    _check(_lib.tddft_workspace_bytes(ctx._h, C.byref(n)), ctx._h)
+    return n.value
+
+
+def tddft_apply_liouville(ctx, X, AX, nvec, mode=TDDFT_SPIN_CONSERVING):
+    """X, AX: CUDA torch tensors complex128 [nvec, vector_len] (AX is written)."""
+    _check(_lib.tddft_apply_liouville(ctx._h, _ptr(X), _ptr(AX), C.c_int(nvec), C.c_int(mode)), ctx._h)
+
+
+def tddft_apply_liouville_host(ctx, X_host, AX_host, nvec, mode=TDDFT_SPIN_CONSERVING):
+    """X_host, AX_host: numpy complex128 arrays or (pinned) CPU torch tensors."""
+    def hp(a):
+        return C.c_void_p(a.ctypes.data) if isinstance(a, np.ndarray) else C.c_void_p(a.data_ptr())
+    _check(_lib.tddft_apply_liouville_host(ctx._h, hp(X_host), hp(AX_host), C.c_int(nvec), C.c_int(mode)), ctx._h)
+
+
+def tddft_davidson(ctx, nroots, mode=TDDFT_SPIN_CONSERVING, evecs=None, allow_unconverged=False):
+    """Returns (evals[nroots], iters, resnorms[nroots]); evecs: optional CUDA tensor [nroots, vector_len]."""
+    ev = np.zeros(nroots, dtype=np.float64)
+    rn = np.zeros(nroots, dtype=np.float64)
+    it = C.c_int(0)
+    rc = _lib.tddft_davidson(ctx._h, C.c_int(nroots), C.c_int(mode), ev.ctypes.data_as(C.c_void_p), _ptr(evecs),
+                             C.byref(it), rn.ctypes.data_as(C.c_void_p))
+    if not (allow_unconverged and rc == TDDFT_ENOTCONVERGED):
+        _check(rc, ctx._h)
+    return ev, it.value, rn
+
+
+def tddft_set_timing(ctx, enabled):
+    _check(_lib.tddft_set_timing(ctx._h, C.c_int(1 if enabled else 0)), ctx._h)
+
+
+def tddft_get_stats(ctx):
+    s = tddft_stats()
+    _check(_lib.tddft_get_stats(ctx._h, C.byref(s)), ctx._h)
+    return {k: getattr(s, k) for k, _ in tddft_stats._fields_}
+
+
+def tddft_pair_potentials(ctx, spin, pairs, tau):
+    p = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+    _check(_lib.tddft_pair_potentials(ctx._h, C.c_int(spin), p.ctypes.data_as(C.c_void_p), C.c_long(len(p)), _ptr(tau)), ctx._h)
+
+
+def tddft_project(ctx, spin, Y, nfun):
+    _check(_lib.tddft_project(ctx._h, C.c_int(spin), _ptr(Y), C.c_long(nfun)), ctx._h)
+
+
+def tddft_gram(ctx, V, W, m, n_complex):
+    G = np.zeros((m, m), dtype=np.float64)
+    _check(_lib.tddft_gram(ctx._h, _ptr(V), _ptr(W), C.c_int(m), C.c_long(n_complex), G.ctypes.data_as(C.c_void_p)), ctx._h)
+    return G
+
+
+def tddft_orbital_real_space(ctx, spin, v, out):
+    _check(_lib.tddft_orbital_real_space(ctx._h, C.c_int(spin), C.c_int(v), _ptr(out)), ctx._h)
+
+
+def tddft_last_error(ctx=None):
+    msg = _lib.tddft_last_error(None if ctx is None else ctx._h)
+    return msg.decode() if msg else ""
+
+
+def tddft_destroy(ctx):
+    ctx.destroy()

@@ -1,0 +1,523 @@
+// C ABI of the library and the driver of one Liouville application.
+// Product path: every numerical step below is a kernel launch; the host only orchestrates.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include "ctx.h"
+
+using namespace tddft;
+
+static std::string g_init_error;
+
+namespace tddft {
+
+int set_err(tddft_ctx* c, int status, const std::string& msg) {
+    if (c) c->err = msg; else g_init_error = msg;
+    return status;
+}
+
+long vector_len(const tddft_ctx* c, int mode) {
+    if (mode == TDDFT_SPIN_CONSERVING) {
+        long n = 0;
+        for (int s = 0; s < c->nspin; ++s) n += (long)c->nocc[s] * c->hp.npwh;
+        return n;
+    }
+    if (c->nspin != 2) return -1;
+    return (long)c->nocc[mode == TDDFT_SPIN_FLIP ? 0 : 1] * c->hp.npwh;
+}
+
+int ensure_arena(tddft_ctx* c, size_t bytes) {
+    if (bytes <= c->arena_bytes) return TDDFT_OK;
+    if (c->arena) { cudaFree(c->arena); c->arena = nullptr; c->arena_bytes = 0; }
+    cudaError_t e = cudaMalloc((void**)&c->arena, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return set_err(c, TDDFT_ENOMEM, "device workspace allocation failed"); }
+    c->arena_bytes = bytes;
+    return TDDFT_OK;
+}
+
+// ---- stage timing ---------------------------------------------------------------------------------
+enum { ST_S1 = 0, ST_S23, ST_S4, ST_S5, ST_S6, ST_S8, ST_COUNT };
+struct StageTimer {
+    tddft_ctx* c; int idx = -1;
+    StageTimer(tddft_ctx* c_, int stage) : c(c_) {
+        if (!c->timing) return;
+        StageEvent ev; ev.stage = stage;
+        cudaEventCreate(&ev.beg); cudaEventCreate(&ev.end);
+        cudaEventRecord(ev.beg, c->stream);
+        c->events.push_back(ev); idx = (int)c->events.size() - 1;
+    }
+    ~StageTimer() { if (idx >= 0) cudaEventRecord(c->events[idx].end, c->stream); }
+};
+static void collect_timing(tddft_ctx* c) {
+    if (!c->timing) return;
+    cudaStreamSynchronize(c->stream);
+    double ms[ST_COUNT] = {0};
+    for (auto& ev : c->events) {
+        float t = 0; cudaEventElapsedTime(&t, ev.beg, ev.end);
+        ms[ev.stage] += t;
+        cudaEventDestroy(ev.beg); cudaEventDestroy(ev.end);
+    }
+    c->events.clear();
+    c->stats.ms_s1_to_real = ms[ST_S1]; c->stats.ms_s23_hxc = ms[ST_S23]; c->stats.ms_s4_pair_fft = ms[ST_S4];
+    c->stats.ms_s5_contract = ms[ST_S5]; c->stats.ms_s6_to_sphere = ms[ST_S6]; c->stats.ms_s8_project = ms[ST_S8];
+    c->stats.ms_total = 0; for (int i = 0; i < ST_COUNT; ++i) c->stats.ms_total += ms[i];
+}
+
+// ---- FFT pass sequences ---------------------------------------------------------------------------
+static SArgs ypass_args(const tddft_ctx* c, int batch) {
+    const int* n = c->hp.n;
+    SArgs a{}; a.n = n[1]; a.stride = n[2]; a.inner = n[2]; a.nouter = n[0]; a.outer_stride = (long)n[1] * n[2];
+    a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[1]; a.work = c->d_work; a.ktab = nullptr;
+    return a;
+}
+static SArgs xpass_args(const tddft_ctx* c, int batch) {
+    const int* n = c->hp.n;
+    SArgs a{}; a.n = n[0]; a.stride = (long)n[1] * n[2]; a.inner = (long)n[1] * n[2]; a.nouter = 1; a.outer_stride = 0;
+    a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc;
+    return a;
+}
+static ZArgs zpass_args(const tddft_ctx* c, int batch) {
+    const int* n = c->hp.n;
+    ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.work = c->d_work;
+    a.lscale = 1.0; a.sscale = 1.0;
+    return a;
+}
+
+// tau_p = C[phi_i phi_j] for npairs pairs (device list), two pairs per complex grid
+static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, long npairs, double* tau) {
+    const long nr = c->hp.nr;
+    for (long p0 = 0; p0 < npairs; p0 += 2L * c->fft_batch) {
+        const int np = (int)std::min<long>(2L * c->fft_batch, npairs - p0);
+        const int nb = (np + 1) / 2;
+        ZArgs z = zpass_args(c, nb);
+        z.phi = phi; z.pairs = d_pairs + p0; z.npairs = np;
+        TD_CUDA(c, launch_zpass(false, ZL_PAIR, ZS_WORK, z, c->stream));
+        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        z.dst = tau + p0 * nr; z.nfun = np; z.sscale = 1.0;
+        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
+        c->stats.kernel_launches += 5;
+        c->stats.pair_ffts += np;
+    }
+    return TDDFT_OK;
+}
+
+// S1: nfun half-sphere functions -> real space, dst[f][r] = Omega^-1/2 sum_G c_f(G) exp(i G.r)
+static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst) {
+    const long nr = c->hp.nr;
+    const double scale = 1.0 / std::sqrt(c->hp.omega);
+    for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
+        const int nf = std::min(2 * c->fft_batch, nfun - f0);
+        const int nb = (nf + 1) / 2;
+        TD_CUDA(c, launch_scatter_pack2(X, lay, f0, nfun, nb, c->d_idx_p, c->d_idx_m, c->d_work, nr, c->stream));
+        TD_CUDA(c, launch_spass(SM_INV, xpass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        ZArgs z = zpass_args(c, nb);
+        z.dst = dst + (long)f0 * nr; z.nfun = nf; z.sscale = scale;
+        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
+        c->stats.kernel_launches += 4;
+    }
+    return TDDFT_OK;
+}
+
+// S6+S7: real-space functions -> half sphere, AX = (Omega^1/2/N_r) FFT[src] + (|G|^2/2 - eps_v) X
+static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig) {
+    const long nr = c->hp.nr;
+    const double scale = std::sqrt(c->hp.omega) / (double)nr;
+    for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
+        const int nf = std::min(2 * c->fft_batch, nfun - f0);
+        const int nb = (nf + 1) / 2;
+        ZArgs z = zpass_args(c, nb);
+        z.src0 = src + (long)f0 * nr; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0;
+        TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
+        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_FWD, xpass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_gather_unpack2(c->d_work, nr, c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream));
+        c->stats.kernel_launches += 4;
+    }
+    return TDDFT_OK;
+}
+
+// S3 Hartree part: vh[kk] = C[scale * (d0[kk] + d1[kk])]
+static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scale, int kc, double* vh) {
+    const long nr = c->hp.nr;
+    for (int f0 = 0; f0 < kc; f0 += 2 * c->fft_batch) {
+        const int nf = std::min(2 * c->fft_batch, kc - f0);
+        const int nb = (nf + 1) / 2;
+        ZArgs z = zpass_args(c, nb);
+        z.src0 = d0 + (long)f0 * nr; z.src1 = d1 ? d1 + (long)f0 * nr : nullptr; z.nfun = nf; z.lscale = scale;
+        TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
+        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
+        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        z.dst = vh + (long)f0 * nr; z.sscale = 1.0;
+        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
+        c->stats.kernel_launches += 5;
+    }
+    return TDDFT_OK;
+}
+
+// S8: rows <- P_c rows with the occupied orbitals of tgt_spin, two tensor-core GEMMs
+int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_stride, double* O) {
+    const long k2 = 2 * c->hp.npwh;
+    const int no = c->nocc[tgt];
+    TD_CUDA(c, launch_gemm_nt(c->psi[tgt], k2, Y, k2, grp, grp_stride, O, nrows, no, nrows, k2, k2, 2.0, 1, nullptr, c->stream));
+    TD_CUDA(c, launch_gemm_tn_acc(O, nrows, c->psi[tgt], k2, Y, k2, grp, grp_stride, nrows, k2, no, -1.0, c->stream));
+    c->stats.kernel_launches += 2;
+    return TDDFT_OK;
+}
+
+// ---- pair tiles -------------------------------------------------------------------------------------
+static int build_tiles(tddft_ctx* c, int spin, int T) {
+    PairTiles& pt = c->tiles[spin];
+    const int N = c->nocc[spin];
+    if (pt.T == T && pt.nocc == N && pt.d_pairs) return TDDFT_OK;
+    if (pt.d_pairs) cudaFree(pt.d_pairs);
+    if (pt.d_slot) cudaFree(pt.d_slot);
+    pt = PairTiles{};
+    pt.T = T; pt.nocc = N;
+    const int nb = (N + T - 1) / T;
+    std::vector<int2> pairs; std::vector<int> slot;
+    for (int bi = 0; bi < nb; ++bi)
+        for (int bj = bi; bj < nb; ++bj) {
+            TileInfo t{};
+            t.i0 = bi * T; t.ti = std::min(T, N - t.i0); t.j0 = bj * T; t.tj = std::min(T, N - t.j0);
+            t.pair_off = (long)pairs.size(); t.slot_off = (long)slot.size();
+            std::vector<int> s((size_t)t.ti * t.tj, -1);
+            int cnt = 0;
+            for (int i = 0; i < t.ti; ++i)
+                for (int j = 0; j < t.tj; ++j) {
+                    const int gi = t.i0 + i, gj = t.j0 + j;
+                    if (gi > gj) continue;
+                    pairs.push_back(make_int2(gi, gj));
+                    s[(size_t)i * t.tj + j] = cnt++;
+                }
+            if (bi == bj) for (int i = 0; i < t.ti; ++i) for (int j = 0; j < i; ++j) s[(size_t)i * t.tj + j] = s[(size_t)j * t.tj + i];
+            t.npairs = cnt;
+            slot.insert(slot.end(), s.begin(), s.end());
+            t.slotT_off = -1;
+            if (bi != bj) {
+                t.slotT_off = (long)slot.size();
+                for (int j = 0; j < t.tj; ++j) for (int i = 0; i < t.ti; ++i) slot.push_back(s[(size_t)i * t.tj + j]);
+            }
+            pt.max_pairs = std::max<long>(pt.max_pairs, cnt);
+            pt.tiles.push_back(t);
+        }
+    TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * pairs.size()));
+    TD_CUDA(c, cudaMalloc((void**)&pt.d_slot, sizeof(int) * slot.size()));
+    TD_CUDA(c, cudaMemcpyAsync(pt.d_pairs, pairs.data(), sizeof(int2) * pairs.size(), cudaMemcpyHostToDevice, c->stream));
+    TD_CUDA(c, cudaMemcpyAsync(pt.d_slot, slot.data(), sizeof(int) * slot.size(), cudaMemcpyHostToDevice, c->stream));
+    TD_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors go out of scope
+    return TDDFT_OK;
+}
+
+// ---- one application ------------------------------------------------------------------------------
+struct Block { int src, tgt; long off; };   // occupied spin, target spin, offset (complex) inside a trial vector
+
+int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, int mode) {
+    if (!c) return TDDFT_EINVAL;
+    if (!Xd || !AXd || nvec < 1) return set_err(c, TDDFT_EINVAL, "apply: null buffer or nvec < 1");
+    if (Xd == AXd) return set_err(c, TDDFT_EINVAL, "apply: AX must not alias X");
+    if (mode < 0 || mode > 2) return set_err(c, TDDFT_EINVAL, "apply: unknown mode");
+    if (mode != TDDFT_SPIN_CONSERVING && c->nspin != 2) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    const cplx* X = (const cplx*)Xd; cplx* AX = (cplx*)AXd;
+    const long nr = c->hp.nr, npwh = c->hp.npwh, L = vector_len(c, mode);
+    c->stats = tddft_stats{};
+    std::vector<Block> blocks;
+    if (mode == TDDFT_SPIN_CONSERVING) { long off = 0; for (int s = 0; s < c->nspin; ++s) { blocks.push_back({s, s, off}); off += (long)c->nocc[s] * npwh; } }
+    else { const int src = (mode == TDDFT_SPIN_FLIP) ? 0 : 1; blocks.push_back({src, 1 - src, 0}); }
+    const bool hxc = (mode == TDDFT_SPIN_CONSERVING) && c->use_hartree_fxc;
+    int maxocc = 0, sumocc = 0;
+    for (auto& b : blocks) { maxocc = std::max(maxocc, c->nocc[b.src]); sumocc += c->nocc[b.src]; }
+
+    // ---- workspace plan: k chunk kc and tile edge T under the budget --------------------------------
+    size_t budget;
+    {
+        size_t fr = 0, tot = 0; cudaMemGetInfo(&fr, &tot);
+        budget = (size_t)(0.85 * (double)(fr + c->arena_bytes));
+        if (c->workspace_gb > 0) budget = std::min(budget, (size_t)(c->workspace_gb * 1073741824.0));
+    }
+    int kc = nvec, T = 0;
+    size_t fixed = 0;
+    const size_t grid_b = sizeof(double) * (size_t)nr;
+    for (;;) {
+        fixed = grid_b * (size_t)kc * ((size_t)sumocc + (size_t)maxocc + (hxc ? 2 * blocks.size() + 1 : 0))
+              + sizeof(double) * (size_t)maxocc * (size_t)kc * (size_t)maxocc + 4096;
+        T = (c->pair_tile > 0) ? std::min(c->pair_tile, maxocc) : std::min(maxocc, 128);
+        const int tmin = std::min(maxocc, 16);
+        while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 8);
+        if (fixed + grid_b * (size_t)T * T <= budget) break;
+        if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
+        kc = (kc + 1) / 2;
+    }
+    { const int nbk = (maxocc + T - 1) / T; T = (maxocc + nbk - 1) / nbk; }   // balance the blocks
+    int rc = ensure_arena(c, fixed + grid_b * (size_t)T * T);
+    if (rc) return rc;
+    char* p = c->arena;
+    auto carve = [&](size_t bytes) { char* q = p; p += (bytes + 255) / 256 * 256; return (double*)q; };
+    std::vector<double*> a(blocks.size());
+    for (size_t b = 0; b < blocks.size(); ++b) a[b] = carve(grid_b * (size_t)kc * c->nocc[blocks[b].src]);
+    double* out = carve(grid_b * (size_t)kc * maxocc);
+    std::vector<double*> drho(blocks.size(), nullptr), V(blocks.size(), nullptr);
+    double* vh = nullptr;
+    if (hxc) { for (size_t b = 0; b < blocks.size(); ++b) { drho[b] = carve(grid_b * kc); V[b] = carve(grid_b * kc); } vh = carve(grid_b * kc); }
+    double* O = carve(sizeof(double) * (size_t)maxocc * kc * maxocc);
+    double* tau = carve(grid_b * (size_t)T * T);
+    for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src])); if (rc) return rc; }
+
+    for (int k0 = 0; k0 < nvec; k0 += kc) {
+        const int kcc = std::min(kc, nvec - k0);
+        // S1 (+S2): trial functions to real space, response densities
+        for (size_t b = 0; b < blocks.size(); ++b) {
+            const int no = c->nocc[blocks[b].src];
+            FunLayout lay{L, blocks[b].off, npwh, kcc, k0};
+            { StageTimer t(c, ST_S1); rc = to_real_space(c, X, lay, no * kcc, a[b]); if (rc) return rc; }
+            if (hxc) { StageTimer t(c, ST_S23); TD_CUDA(c, launch_drho(c->d_phi[blocks[b].src], a[b], no, kcc, nr, drho[b], c->stream)); c->stats.kernel_launches += (kcc + 3) / 4; }
+        }
+        // S3: Hartree + f_xc potential (Eq. 4 with f_Hxc = v_c + f_xc)
+        if (hxc) {
+            StageTimer t(c, ST_S23);
+            if (c->nspin == 2) {
+                rc = hartree(c, drho[0], drho[1], 1.0, kcc, vh); if (rc) return rc;
+                TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[0], drho[0], c->d_fxc[1], drho[1], kcc, nr, V[0], c->stream));
+                TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[1], drho[0], c->d_fxc[2], drho[1], kcc, nr, V[1], c->stream));
+                c->stats.kernel_launches += 2;
+            } else {   // closed shell, singlet channel (reading A6): V = C[2 drho] + (f_uu + f_ud) drho
+                rc = hartree(c, drho[0], nullptr, 2.0, kcc, vh); if (rc) return rc;
+                TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[0], drho[0], c->d_fxc[1], drho[0], kcc, nr, V[0], c->stream));
+                c->stats.kernel_launches += 1;
+            }
+        }
+        for (size_t b = 0; b < blocks.size(); ++b) {
+            const Block& bl = blocks[b];
+            const int no = c->nocc[bl.src];
+            const double* phi = c->d_phi[bl.src];
+            { StageTimer t(c, ST_S5);
+              TD_CUDA(c, launch_out_init(phi, hxc ? V[b] : nullptr, c->vloc[bl.tgt], a[b], no, kcc, nr, out, c->stream)); c->stats.kernel_launches += 1; }
+            // S4 + S5: exact-exchange response, tile by tile (Eq. 6; tau_vv' of PAPER.md:230)
+            if (c->alpha != 0.0) {
+                const PairTiles& pt = c->tiles[bl.src];
+                for (const TileInfo& t : pt.tiles) {
+                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, t.npairs, tau); if (rc) return rc; }
+                    StageTimer tm(c, ST_S5);
+                    TD_CUDA(c, launch_contract(out, a[b], tau, pt.d_slot + t.slot_off, t.i0, t.ti, t.j0, t.tj, kcc, nr, c->alpha, c->stream));
+                    c->stats.kernel_launches += 1;
+                    if (t.slotT_off >= 0) {
+                        TD_CUDA(c, launch_contract(out, a[b], tau, pt.d_slot + t.slotT_off, t.j0, t.tj, t.i0, t.ti, kcc, nr, c->alpha, c->stream));
+                        c->stats.kernel_launches += 1;
+                    }
+                }
+            }
+            // S6 + S7: back to the sphere, add D (Eq. 3 with the model H of reading A4)
+            FunLayout lay{L, bl.off, npwh, kcc, k0};
+            { StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, X, AX, lay, c->d_eig[bl.src]); if (rc) return rc; }
+            // S8: conduction-band projector of the target spin
+            { StageTimer t(c, ST_S8);
+              rc = project_rows(c, bl.tgt, (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, O); if (rc) return rc; }
+        }
+    }
+    collect_timing(c);
+    return TDDFT_OK;
+}
+
+}  // namespace tddft
+
+// =====================================================================================================
+extern "C" {
+#pragma GCC visibility push(default)
+
+int tddft_enumerate_gvectors(const double* lattice, double ecut, long capacity, int* miller, double* g2, long* npwh) {
+    if (!lattice || !npwh || !(ecut > 0)) return TDDFT_EINVAL;
+    try {
+        std::vector<int> m; std::vector<double> q;
+        const long n = enumerate_half_sphere(lattice, ecut, &m, &q);
+        *npwh = n;
+        if ((miller || g2) && capacity < n) return TDDFT_EINVAL;
+        if (miller) std::memcpy(miller, m.data(), sizeof(int) * 3 * n);
+        if (g2) std::memcpy(g2, q.data(), sizeof(double) * n);
+    } catch (const std::bad_alloc&) { return TDDFT_ENOMEM; }
+    return TDDFT_OK;
+}
+
+int tddft_destroy(tddft_ctx* c) {
+    if (!c) return TDDFT_OK;
+    cudaFree(c->d_idx_p); cudaFree(c->d_idx_m); cudaFree(c->d_kin); cudaFree(c->d_vc);
+    for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
+    for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
+    cudaFree(c->d_work); cudaFree(c->arena);
+    for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); }
+    cudaGetLastError();
+    delete c;
+    return TDDFT_OK;
+}
+
+int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double ecut, int nspin, const int* nocc,
+               const double* psi_up, const double* psi_dn, const double* eig_up, const double* eig_dn, double alpha,
+               const tddft_options* opt) {
+    if (!out) return TDDFT_EINVAL;
+    *out = nullptr;
+    if (!lattice || !grid || !nocc || !psi_up || !eig_up) return set_err(nullptr, TDDFT_EINVAL, "init: null argument");
+    if (nspin != 1 && nspin != 2) return set_err(nullptr, TDDFT_EINVAL, "init: nspin must be 1 or 2");
+    if (nspin == 2 && (!psi_dn || !eig_dn)) return set_err(nullptr, TDDFT_EINVAL, "init: nspin = 2 needs psi_dn and eig_dn");
+    if (!(ecut > 0) || !(alpha >= 0)) return set_err(nullptr, TDDFT_EINVAL, "init: ecut must be > 0 and alpha >= 0");
+    for (int s = 0; s < nspin; ++s) if (nocc[s] < 1) return set_err(nullptr, TDDFT_EINVAL, "init: nocc must be >= 1");
+    for (int a = 0; a < 3; ++a) if (grid[a] < 1) return set_err(nullptr, TDDFT_EINVAL, "init: bad grid");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return set_err(nullptr, TDDFT_ECUDA, "init: no CUDA device (this library has no CPU path)"); }
+    tddft_ctx* c = nullptr;
+    try { c = new tddft_ctx(); } catch (const std::bad_alloc&) { return TDDFT_ENOMEM; }
+    auto fail = [&](int st, const std::string& msg) { g_init_error = msg; tddft_destroy(c); return st; };
+    try {
+        for (int a = 0; a < 3; ++a) if (!fft_size_supported(grid[a])) return fail(TDDFT_EUNSUPPORTED, "init: FFT length without a plan");
+        const char* perr = build_host_plan(lattice, grid, ecut, &c->hp);
+        if (perr) return fail(std::strstr(perr, "plan") ? TDDFT_EUNSUPPORTED : TDDFT_EINVAL, std::string("init: ") + perr);
+        c->ecut = ecut; c->alpha = alpha; c->nspin = nspin;
+        c->nocc[0] = nocc[0]; c->nocc[1] = nspin == 2 ? nocc[1] : 0;
+        c->psi[0] = psi_up; c->psi[1] = nspin == 2 ? psi_dn : nullptr;
+        c->eig_h[0].assign(eig_up, eig_up + nocc[0]);
+        if (nspin == 2) c->eig_h[1].assign(eig_dn, eig_dn + nocc[1]);
+        if (opt) {
+            if (opt->struct_size != (int)sizeof(tddft_options)) return fail(TDDFT_EINVAL, "init: tddft_options.struct_size mismatch");
+            if (opt->use_hartree_fxc >= 0) c->use_hartree_fxc = opt->use_hartree_fxc ? 1 : 0;
+            if (opt->rho_floor > 0) c->rho_floor = opt->rho_floor;
+            c->vloc[0] = opt->vloc_up; c->vloc[1] = nspin == 2 ? opt->vloc_dn : nullptr;
+            c->stream = (cudaStream_t)opt->cuda_stream;
+            c->workspace_gb = opt->workspace_gb; c->pair_tile = opt->pair_tile; c->fft_batch = opt->fft_batch;
+            c->dav_max_subspace = opt->max_subspace; c->dav_max_iter = opt->max_iter; c->dav_tol = opt->tol;
+            c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
+        }
+        const long nr = c->hp.nr, npwh = c->hp.npwh;
+        if (c->fft_batch <= 0) c->fft_batch = (int)std::max<long>(1, std::min<long>(64, (64L << 20) / (16 * nr)));
+#define INIT_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? TDDFT_ENOMEM : TDDFT_ECUDA, std::string("init: " #call ": ") + cudaGetErrorString(e_)); } while (0)
+        INIT_CUDA(cudaMalloc((void**)&c->d_idx_p, sizeof(int) * npwh));
+        INIT_CUDA(cudaMalloc((void**)&c->d_idx_m, sizeof(int) * npwh));
+        INIT_CUDA(cudaMalloc((void**)&c->d_kin, sizeof(double) * npwh));
+        INIT_CUDA(cudaMalloc((void**)&c->d_vc, sizeof(double) * nr));
+        INIT_CUDA(cudaMalloc((void**)&c->d_work, sizeof(cplx) * nr * c->fft_batch));
+        std::vector<double> kin(npwh);
+        for (long g = 0; g < npwh; ++g) kin[g] = 0.5 * c->hp.g2[g];
+        INIT_CUDA(cudaMemcpy(c->d_idx_p, c->hp.idx_p.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_idx_m, c->hp.idx_m.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_kin, kin.data(), sizeof(double) * npwh, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_vc, c->hp.vc.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
+        for (int a = 0; a < 3; ++a) {
+            const int n = grid[a];
+            std::vector<cplx> tw(n);
+            for (int k = 0; k < n; ++k) {   // exp(-2 pi i k/n), argument reduced exactly, long double sincos
+                const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)n;
+                tw[k] = make_double2((double)cosl(ang), (double)sinl(ang));
+            }
+            INIT_CUDA(cudaMalloc((void**)&c->d_tw[a], sizeof(cplx) * n));
+            INIT_CUDA(cudaMemcpy(c->d_tw[a], tw.data(), sizeof(cplx) * n, cudaMemcpyHostToDevice));
+        }
+        for (int s = 0; s < nspin; ++s) {
+            INIT_CUDA(cudaMalloc((void**)&c->d_eig[s], sizeof(double) * c->nocc[s]));
+            INIT_CUDA(cudaMemcpy(c->d_eig[s], c->eig_h[s].data(), sizeof(double) * c->nocc[s], cudaMemcpyHostToDevice));
+            INIT_CUDA(cudaMalloc((void**)&c->d_phi[s], sizeof(double) * nr * c->nocc[s]));
+            FunLayout lay{0, 0, npwh, 1, 0};
+            int rc = to_real_space(c, (const cplx*)c->psi[s], lay, c->nocc[s], c->d_phi[s]);
+            if (rc) { std::string m = c->err; return fail(rc, m); }
+        }
+        // rho0 and LDA f_xc (Eq. 8)
+        for (int a = 0; a < 3; ++a) INIT_CUDA(cudaMalloc((void**)&c->d_fxc[a], sizeof(double) * nr));
+        {
+            double *ru = nullptr, *rd = nullptr;
+            INIT_CUDA(cudaMalloc((void**)&ru, sizeof(double) * nr));
+            INIT_CUDA(launch_rho0(c->d_phi[0], c->nocc[0], nr, ru, c->stream));
+            if (nspin == 2) { INIT_CUDA(cudaMalloc((void**)&rd, sizeof(double) * nr)); INIT_CUDA(launch_rho0(c->d_phi[1], c->nocc[1], nr, rd, c->stream)); }
+            INIT_CUDA(launch_lda_fxc(ru, nspin == 2 ? rd : ru, nr, c->rho_floor, c->d_fxc[0], c->d_fxc[1], c->d_fxc[2], c->stream));
+            INIT_CUDA(cudaStreamSynchronize(c->stream));
+            cudaFree(ru); cudaFree(rd);
+        }
+#undef INIT_CUDA
+    } catch (const std::bad_alloc&) { return fail(TDDFT_ENOMEM, "init: host allocation failed"); }
+    c->stats = tddft_stats{};
+    *out = c;
+    return TDDFT_OK;
+}
+
+int tddft_npw_half(const tddft_ctx* c, long* npwh) { if (!c || !npwh) return TDDFT_EINVAL; *npwh = c->hp.npwh; return TDDFT_OK; }
+int tddft_gvectors(const tddft_ctx* c, int* miller) {
+    if (!c || !miller) return TDDFT_EINVAL;
+    std::memcpy(miller, c->hp.miller.data(), sizeof(int) * 3 * c->hp.npwh);
+    return TDDFT_OK;
+}
+int tddft_vector_len(const tddft_ctx* c, int mode, long* n) {
+    if (!c || !n || mode < 0 || mode > 2) return TDDFT_EINVAL;
+    const long v = vector_len(c, mode);
+    if (v < 0) return TDDFT_EINVAL;
+    *n = v; return TDDFT_OK;
+}
+int tddft_workspace_bytes(const tddft_ctx* c, long long* bytes) { if (!c || !bytes) return TDDFT_EINVAL; *bytes = (long long)c->arena_bytes; return TDDFT_OK; }
+
+int tddft_apply_liouville(tddft_ctx* c, const double* X, double* AX, int nvec, int mode) {
+    try { return apply_liouville_dev(c, X, AX, nvec, mode); }
+    catch (const std::bad_alloc&) { return set_err(c, TDDFT_ENOMEM, "apply: host allocation failed"); }
+}
+
+int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int nvec, int mode) {
+    if (!c || !Xh || !AXh || nvec < 1 || mode < 0 || mode > 2) return TDDFT_EINVAL;
+    const long L = vector_len(c, mode);
+    if (L < 0) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    const size_t bytes = sizeof(cplx) * (size_t)L * nvec;
+    double *dX = nullptr, *dAX = nullptr;
+    if (cudaMalloc((void**)&dX, bytes) != cudaSuccess || cudaMalloc((void**)&dAX, bytes) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(dX); return set_err(c, TDDFT_ENOMEM, "apply_host: device allocation failed");
+    }
+    int rc = TDDFT_OK;
+    if (cudaMemcpyAsync(dX, Xh, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: H2D copy failed");
+    if (!rc) rc = tddft_apply_liouville(c, dX, dAX, nvec, mode);
+    if (!rc && cudaMemcpyAsync(AXh, dAX, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && !rc) rc = set_err(c, TDDFT_ECUDA, "apply_host: stream failed");
+    cudaFree(dX); cudaFree(dAX);
+    return rc;
+}
+
+int tddft_set_timing(tddft_ctx* c, int enabled) { if (!c) return TDDFT_EINVAL; c->timing = enabled != 0; return TDDFT_OK; }
+int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) { if (!c || !out) return TDDFT_EINVAL; *out = c->stats; return TDDFT_OK; }
+
+int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs, double* tau) {
+    if (!c || !pairs || !tau || n_pairs < 0 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
+    for (long i = 0; i < 2 * n_pairs; ++i) if (pairs[i] < 0 || pairs[i] >= c->nocc[spin]) return set_err(c, TDDFT_EINVAL, "pair index out of range");
+    if (n_pairs == 0) return TDDFT_OK;
+    int2* d = nullptr;
+    TD_CUDA(c, cudaMalloc((void**)&d, sizeof(int2) * n_pairs));
+    cudaError_t e = cudaMemcpyAsync(d, pairs, sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, c->stream);
+    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, n_pairs, tau) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
+    cudaStreamSynchronize(c->stream);
+    cudaFree(d);
+    return rc;
+}
+
+int tddft_project(tddft_ctx* c, int spin, double* Y, long nfun) {
+    if (!c || !Y || nfun < 1 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
+    int rc = ensure_arena(c, sizeof(double) * (size_t)c->nocc[spin] * nfun);
+    if (rc) return rc;
+    return project_rows(c, spin, Y, (int)nfun, (int)nfun, 0, (double*)c->arena);
+}
+
+int tddft_gram(tddft_ctx* c, const double* V, const double* W, int m, long n_complex, double* G) {
+    if (!c || !V || !W || !G || m < 1 || n_complex < 1) return TDDFT_EINVAL;
+    const long K = 2 * n_complex;
+    int splits = (int)std::max<long>(1, std::min<long>(1024, K / 8192));
+    int rc = ensure_arena(c, sizeof(double) * (size_t)m * m * (splits + 1));
+    if (rc) return rc;
+    double* part = (double*)c->arena; double* Gd = part + (size_t)m * m * splits;
+    TD_CUDA(c, launch_gemm_nt(V, K, W, K, m, 0, Gd, m, m, m, K, 2 * c->hp.npwh, 2.0, splits, part, c->stream));
+    TD_CUDA(c, cudaMemcpyAsync(G, Gd, sizeof(double) * m * m, cudaMemcpyDeviceToHost, c->stream));
+    TD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return TDDFT_OK;
+}
+
+int tddft_orbital_real_space(tddft_ctx* c, int spin, int v, double* out) {
+    if (!c || !out || spin < 0 || spin >= c->nspin || v < 0 || v >= c->nocc[spin]) return TDDFT_EINVAL;
+    TD_CUDA(c, cudaMemcpyAsync(out, c->d_phi[spin] + (long)v * c->hp.nr, sizeof(double) * c->hp.nr, cudaMemcpyDeviceToDevice, c->stream));
+    return TDDFT_OK;
+}
+
+const char* tddft_last_error(const tddft_ctx* c) { return c ? c->err.c_str() : g_init_error.c_str(); }
+
+#pragma GCC visibility pop
+}  // extern "C"

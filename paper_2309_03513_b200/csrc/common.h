@@ -1,0 +1,47 @@
+// Shared declarations of the tddft_b200 library (host side).  Product code: no oracle, no CPU fallback.
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+#include "../../include/tddft.h"
+#include "fft_core.cuh"
+
+namespace tddft {
+
+// ---- FFT pass launchers (fft_inst.cu; one translation unit per size group) ---------------------------
+enum ZLoadKind { ZL_WORK = 0, ZL_PAIR = 1, ZL_PACK2 = 2 };
+enum ZStoreKind { ZS_WORK = 0, ZS_SPLIT2 = 1 };
+
+struct ZArgs {
+    // geometry
+    int n;                 // length of the contiguous axis
+    long npencils;         // pencils per grid (n1*n2)
+    long nr;               // points per grid
+    int batch;             // packed grids in this launch
+    const cplx* tw;        // device twiddles exp(-2 pi i k/n)
+    cplx* work;            // [batch][nr] complex work grids (source for ZL_WORK, destination for ZS_WORK)
+    // ZL_PAIR: packed grid b = phi[pairs[2b].x]*phi[pairs[2b].y] + i phi[pairs[2b+1].x]*phi[pairs[2b+1].y]
+    const double* phi;     // [norb][nr]
+    const int2* pairs;     // device, npairs entries (already offset to this launch)
+    int npairs;
+    // ZL_PACK2: re = scale*(src0[2b] + src1[2b]), im = same for 2b+1 (src1 optional); nfun functions
+    const double* src0;
+    const double* src1;
+    double lscale;
+    // ZS_SPLIT2: dst[2b] = sscale*re, dst[2b+1] = sscale*im  (nfun functions; pairs mode uses npairs)
+    double* dst;
+    int nfun;
+    double sscale;
+};
+// strided passes along an axis with element stride `stride` over `inner` contiguous elements, `nouter` slabs
+enum SMode { SM_FWD = 0, SM_INV = 1, SM_CONV = 2 /* forward, multiply by ktab, inverse */ };
+struct SArgs {
+    int n; long stride; long inner; long nouter; long outer_stride; long nr; int batch;
+    const cplx* tw; cplx* work; const double* ktab;   // ktab [nr] real, same (scrambled) layout as work
+};
+bool fft_size_supported(int n);
+cudaError_t launch_zpass(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st);
+cudaError_t launch_spass(int mode, const SArgs& a, cudaStream_t st);
+void fft_plan_radices(int n, int* r1, int* r2, int* r3);   // 0s if unsupported
+
+}  // namespace tddft

@@ -1,0 +1,70 @@
+// The context behind the C ABI and the internal driver interface shared by api.cu and davidson.cu.
+#pragma once
+#include <string>
+#include <vector>
+#include "common.h"
+#include "kernels.h"
+#include "plan.h"
+
+struct TileInfo {
+    int i0, ti, j0, tj;        // row block [i0, i0+ti), column block [j0, j0+tj), i0 <= j0
+    long pair_off; int npairs; // unique pairs (i <= j) of this tile inside PairTiles::d_pairs
+    long slot_off, slotT_off;  // slot tables [ti][tj] and (off-diagonal tiles) [tj][ti] inside d_slot
+};
+struct PairTiles {
+    int T = 0, nocc = 0;
+    std::vector<TileInfo> tiles;
+    int2* d_pairs = nullptr;
+    int* d_slot = nullptr;
+    long max_pairs = 0;
+};
+
+struct StageEvent { int stage; cudaEvent_t beg, end; };
+
+struct tddft_ctx {
+    tddft::HostPlan hp;
+    double ecut = 0, alpha = 0;
+    int nspin = 1, nocc[2] = {0, 0};
+    const double* psi[2] = {nullptr, nullptr};
+    std::vector<double> eig_h[2];
+    // options
+    int use_hartree_fxc = 1;
+    double rho_floor = 1e-10;
+    const double* vloc[2] = {nullptr, nullptr};
+    cudaStream_t stream = nullptr;
+    double workspace_gb = 0;
+    int pair_tile = 0, fft_batch = 0;
+    int dav_max_subspace = 0, dav_max_iter = 0; double dav_tol = 0; const double* dav_x0 = nullptr; int dav_nx0 = 0;
+    unsigned long long seed = 0;
+    // device tables
+    int *d_idx_p = nullptr, *d_idx_m = nullptr;
+    double *d_kin = nullptr, *d_vc = nullptr, *d_eig[2] = {nullptr, nullptr};
+    tddft::cplx* d_tw[3] = {nullptr, nullptr, nullptr};
+    double* d_phi[2] = {nullptr, nullptr};
+    double* d_fxc[3] = {nullptr, nullptr, nullptr};
+    tddft::cplx* d_work = nullptr;   // [fft_batch][nr]
+    // per-call workspace arena
+    char* arena = nullptr; size_t arena_bytes = 0;
+    PairTiles tiles[2];
+    // bookkeeping
+    tddft_stats stats{};
+    bool timing = false;
+    std::vector<StageEvent> events;
+    std::string err;
+};
+
+namespace tddft {
+int set_err(tddft_ctx* c, int status, const std::string& msg);
+int apply_liouville_dev(tddft_ctx* c, const double* X, double* AX, int nvec, int mode);
+long vector_len(const tddft_ctx* c, int mode);
+// P_c on functions laid out as rows: row n at Y + (n / grp)*grp_stride + (n % grp)*2*npwh (doubles); scratch O from arena
+int project_rows(tddft_ctx* c, int tgt_spin, double* Y, int nrows, int grp, long grp_stride, double* O);
+int ensure_arena(tddft_ctx* c, size_t bytes);
+}  // namespace tddft
+
+#define TD_CUDA(c, call)                                                                                   \
+    do {                                                                                                   \
+        cudaError_t e_ = (call);                                                                           \
+        if (e_ != cudaSuccess)                                                                             \
+            return tddft::set_err((c), TDDFT_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));   \
+    } while (0)

@@ -1,0 +1,49 @@
+// Launch wrappers of the non-FFT kernels (kernels.cu, gemm.cu).  All asynchronous on the given stream.
+#pragma once
+#include <cuda_runtime.h>
+#include "fft_core.cuh"
+
+namespace tddft {
+
+// Where the functions of one spin block of a trial-vector block live: function f = v*kc + kk is the complex
+// half-sphere vector at  base + (k0 + kk)*vec_len + block_off + v*npwh   (units: complex elements).
+struct FunLayout {
+    long vec_len; long block_off; long npwh; int kc; int k0;
+};
+
+// S1: sphere -> zeroed complex work grids, two functions per grid (re/im), functions f0 .. f0+2*batch-1 (< nfun)
+cudaError_t launch_scatter_pack2(const cplx* X, FunLayout lay, int f0, int nfun, int batch, const int* idx_p, const int* idx_m,
+                                 cplx* work, long nr, cudaStream_t st);
+// S6+S7: work grids -> sphere with scale, plus (kin[g] - eig[v]) * x(g)  (Eq. 3)
+cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, const int* idx_m, int f0, int nfun, int batch,
+                                  double scale, const cplx* X, cplx* AX, FunLayout lay, const double* kin, const double* eig,
+                                  cudaStream_t st);
+// plain sphere -> grid for one function per complex grid pair is not needed; orbitals use scatter_pack2 too.
+
+// S2: drho[kk][r] = sum_v phi[v][r] * a[v*kc+kk][r]   (inner sum of Eq. 4)
+cudaError_t launch_drho(const double* phi, const double* a, int nocc, int kc, long nr, double* drho, cudaStream_t st);
+// S3 pointwise: V_s[kk][r] = vh[kk][r] + f_s0[r]*drho0[kk][r] + f_s1[r]*drho1[kk][r]  (drho1/f_s1 may be null)
+cudaError_t launch_hxc_potential(const double* vh, const double* f0, const double* drho0, const double* f1, const double* drho1,
+                                 int kc, long nr, double* V, cudaStream_t st);
+// S5 start value: out[f][r] = phi[v][r]*V[kk][r] (if V) + vloc[r]*a[f][r] (if vloc), f = v*kc+kk
+cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
+                            double* out, cudaStream_t st);
+// S5: out[(i0+i)*kc+kk][r] -= alpha * sum_{j<tj} tau[slot[i*tj+j]][r] * a[(j0+j)*kc+kk][r]   (Eq. 6)
+cudaError_t launch_contract(double* out, const double* a, const double* tau, const int* slot, int i0, int ti, int j0, int tj,
+                            int kc, long nr, double alpha, cudaStream_t st);
+// S0: rho[r] = sum_v phi[v][r]^2 ; LDA kernel f_xc (Eq. 8; reading A5)
+cudaError_t launch_rho0(const double* phi, int nocc, long nr, double* rho, cudaStream_t st);
+cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double* fuu, double* fud,
+                           double* fdd, cudaStream_t st);
+
+// ---- dense contractions on FP64 tensor cores (gemm.cu) ------------------------------------------------
+// C[m][n] (ldc) = cscale * sum_k w_k A[m][k] B[n][k], A rows at lda, B row n at  B + (n / bgrp)*bstride_grp + (n % bgrp)*ldb.
+// w_k = 1/2 where k % wperiod == 0 (wperiod > 0), else 1: with cscale = 2 this is the Gamma-point inner product.
+// K may be split over `splits` CTAs along k; partial sums go to `partial` [splits][m][n] and are reduced in order.
+cudaError_t launch_gemm_nt(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
+                           int M, int N, long K, long wperiod, double cscale, int splits, double* partial, cudaStream_t st);
+// C[m][n] += cscale * sum_k At[k][m] B[k][n];  C row m at  C + (m / cgrp)*cstride_grp + (m % cgrp)*ldc
+cudaError_t launch_gemm_tn_acc(const double* At, long ldat, const double* B, long ldb, double* C, long ldc, int cgrp,
+                               long cstride_grp, int M, long N, int K, double cscale, cudaStream_t st);
+
+}  // namespace tddft

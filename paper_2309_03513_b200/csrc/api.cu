@@ -230,7 +230,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     else { const int src = (mode == TDDFT_SPIN_FLIP) ? 0 : 1; blocks.push_back({src, 1 - src, 0}); }
     const bool hxc = (mode == TDDFT_SPIN_CONSERVING) && c->use_hartree_fxc;
     int maxocc = 0, sumocc = 0;
-    for (auto& b : blocks) { maxocc = std::max(maxocc, c->nocc[b.src]); sumocc += c->nocc[b.src]; }
+    for (auto& b : blocks) { maxocc = std::max(maxocc, std::max(c->nocc[b.src], c->nocc[b.tgt])); sumocc += c->nocc[b.src]; }
 
     // ---- workspace plan: k chunk kc and tile edge T under the budget --------------------------------
     size_t budget;

@@ -85,7 +85,7 @@ static ZArgs zpass_args(const tddft_ctx* c, int batch) {
 }
 
 // tau_p = C[phi_i phi_j] for npairs pairs (device list), two pairs per complex grid
-static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, long npairs, double* tau) {
+static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, long npairs, double* tau, int chunked) {
     const long nr = c->hp.nr;
     for (long p0 = 0; p0 < npairs; p0 += 2L * c->fft_batch) {
         const int np = (int)std::min<long>(2L * c->fft_batch, npairs - p0);
@@ -96,7 +96,7 @@ static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pa
         TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
-        z.dst = tau + p0 * nr; z.nfun = np; z.sscale = 1.0;
+        z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = p0; z.ftotal = npairs;
         TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
         c->stats.kernel_launches += 5;
         c->stats.pair_ffts += np;
@@ -105,7 +105,7 @@ static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pa
 }
 
 // S1: nfun half-sphere functions -> real space, dst[f][r] = Omega^-1/2 sum_G c_f(G) exp(i G.r)
-static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst) {
+static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked) {
     const long nr = c->hp.nr;
     const double scale = 1.0 / std::sqrt(c->hp.omega);
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
@@ -115,7 +115,7 @@ static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, d
         TD_CUDA(c, launch_spass(SM_INV, xpass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
         ZArgs z = zpass_args(c, nb);
-        z.dst = dst + (long)f0 * nr; z.nfun = nf; z.sscale = scale;
+        z.dst = dst; z.nfun = nf; z.sscale = scale; z.chunked = chunked; z.fbase = f0; z.ftotal = nfun;
         TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
         c->stats.kernel_launches += 4;
     }
@@ -130,7 +130,7 @@ static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cpl
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
         const int nb = (nf + 1) / 2;
         ZArgs z = zpass_args(c, nb);
-        z.src0 = src + (long)f0 * nr; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0;
+        z.src0 = src; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0; z.chunked = 1; z.fbase = f0; z.ftotal = nfun;
         TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
         TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_FWD, xpass_args(c, nb), c->stream));
@@ -147,12 +147,12 @@ static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scal
         const int nf = std::min(2 * c->fft_batch, kc - f0);
         const int nb = (nf + 1) / 2;
         ZArgs z = zpass_args(c, nb);
-        z.src0 = d0 + (long)f0 * nr; z.src1 = d1 ? d1 + (long)f0 * nr : nullptr; z.nfun = nf; z.lscale = scale;
+        z.src0 = d0; z.src1 = d1; z.nfun = nf; z.lscale = scale; z.chunked = 0; z.fbase = f0; z.ftotal = kc;
         TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
         TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
         TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
-        z.dst = vh + (long)f0 * nr; z.sscale = 1.0;
+        z.dst = vh; z.sscale = 1.0;
         TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
         c->stats.kernel_launches += 5;
     }
@@ -241,18 +241,18 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     }
     int kc = nvec, T = 0;
     size_t fixed = 0;
-    const size_t grid_b = sizeof(double) * (size_t)nr;
+    const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
     for (;;) {
         fixed = grid_b * (size_t)kc * ((size_t)sumocc + (size_t)maxocc + (hxc ? 2 * blocks.size() + 1 : 0))
               + sizeof(double) * (size_t)maxocc * (size_t)kc * (size_t)maxocc + 4096;
-        T = (c->pair_tile > 0) ? std::min(c->pair_tile, maxocc) : std::min(maxocc, 128);
+        T = std::min(std::min(maxocc, 128), c->pair_tile > 0 ? c->pair_tile : 128);
         const int tmin = std::min(maxocc, 16);
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 8);
         if (fixed + grid_b * (size_t)T * T <= budget) break;
         if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
         kc = (kc + 1) / 2;
     }
-    { const int nbk = (maxocc + T - 1) / T; T = (maxocc + nbk - 1) / nbk; }   // balance the blocks
+    if (T >= 32) T &= ~31;   // the contraction gives each warp 32 rows of a tile
     int rc = ensure_arena(c, fixed + grid_b * (size_t)T * T);
     if (rc) return rc;
     char* p = c->arena;
@@ -273,7 +273,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
         for (size_t b = 0; b < blocks.size(); ++b) {
             const int no = c->nocc[blocks[b].src];
             FunLayout lay{L, blocks[b].off, npwh, kcc, k0};
-            { StageTimer t(c, ST_S1); rc = to_real_space(c, X, lay, no * kcc, a[b]); if (rc) return rc; }
+            { StageTimer t(c, ST_S1); rc = to_real_space(c, X, lay, no * kcc, a[b], 1); if (rc) return rc; }
             if (hxc) { StageTimer t(c, ST_S23); TD_CUDA(c, launch_drho(c->d_phi[blocks[b].src], a[b], no, kcc, nr, drho[b], c->stream)); c->stats.kernel_launches += (kcc + 3) / 4; }
         }
         // S3: Hartree + f_xc potential (Eq. 4 with f_Hxc = v_c + f_xc)
@@ -300,14 +300,11 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
             if (c->alpha != 0.0) {
                 const PairTiles& pt = c->tiles[bl.src];
                 for (const TileInfo& t : pt.tiles) {
-                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, t.npairs, tau); if (rc) return rc; }
+                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, t.npairs, tau, 1); if (rc) return rc; }
                     StageTimer tm(c, ST_S5);
-                    TD_CUDA(c, launch_contract(out, a[b], tau, pt.d_slot + t.slot_off, t.i0, t.ti, t.j0, t.tj, kcc, nr, c->alpha, c->stream));
-                    c->stats.kernel_launches += 1;
-                    if (t.slotT_off >= 0) {
-                        TD_CUDA(c, launch_contract(out, a[b], tau, pt.d_slot + t.slotT_off, t.j0, t.tj, t.i0, t.ti, kcc, nr, c->alpha, c->stream));
-                        c->stats.kernel_launches += 1;
-                    }
+                    if (t.slotT_off >= 0) TD_CUDA(c, launch_contract_dual(out, a[b], tau, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, nr, c->alpha, c->stream));
+                    else TD_CUDA(c, launch_contract_single(out, a[b], tau, pt.d_slot + t.slot_off, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, t.npairs, nr, c->alpha, c->stream));
+                    c->stats.kernel_launches += (kcc + 15) / 16;
                 }
             }
             // S6 + S7: back to the sphere, add D (Eq. 3 with the model H of reading A4)
@@ -346,7 +343,7 @@ int tddft_destroy(tddft_ctx* c) {
     cudaFree(c->d_idx_p); cudaFree(c->d_idx_m); cudaFree(c->d_kin); cudaFree(c->d_vc);
     for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
-    cudaFree(c->d_work); cudaFree(c->arena);
+    cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
     for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); }
     cudaGetLastError();
     delete c;
@@ -396,6 +393,8 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         INIT_CUDA(cudaMalloc((void**)&c->d_kin, sizeof(double) * npwh));
         INIT_CUDA(cudaMalloc((void**)&c->d_vc, sizeof(double) * nr));
         INIT_CUDA(cudaMalloc((void**)&c->d_work, sizeof(cplx) * nr * c->fft_batch));
+        INIT_CUDA(cudaMalloc((void**)&c->d_zeros, 1024));
+        INIT_CUDA(cudaMemset(c->d_zeros, 0, 1024));
         std::vector<double> kin(npwh);
         for (long g = 0; g < npwh; ++g) kin[g] = 0.5 * c->hp.g2[g];
         INIT_CUDA(cudaMemcpy(c->d_idx_p, c->hp.idx_p.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
@@ -417,7 +416,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             INIT_CUDA(cudaMemcpy(c->d_eig[s], c->eig_h[s].data(), sizeof(double) * c->nocc[s], cudaMemcpyHostToDevice));
             INIT_CUDA(cudaMalloc((void**)&c->d_phi[s], sizeof(double) * nr * c->nocc[s]));
             FunLayout lay{0, 0, npwh, 1, 0};
-            int rc = to_real_space(c, (const cplx*)c->psi[s], lay, c->nocc[s], c->d_phi[s]);
+            int rc = to_real_space(c, (const cplx*)c->psi[s], lay, c->nocc[s], c->d_phi[s], 0);
             if (rc) { std::string m = c->err; return fail(rc, m); }
         }
         // rho0 and LDA f_xc (Eq. 8)
@@ -485,7 +484,7 @@ int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs
     int2* d = nullptr;
     TD_CUDA(c, cudaMalloc((void**)&d, sizeof(int2) * n_pairs));
     cudaError_t e = cudaMemcpyAsync(d, pairs, sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, c->stream);
-    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, n_pairs, tau) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
+    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, n_pairs, tau, 0) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
     cudaStreamSynchronize(c->stream);
     cudaFree(d);
     return rc;

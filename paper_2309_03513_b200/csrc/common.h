@@ -32,7 +32,12 @@ struct ZArgs {
     double* dst;
     int nfun;
     double sscale;
+    // layout of the real function batches src0/src1/dst: function index fbase + (0..nfun-1) inside a batch of ftotal
+    // functions; chunked = 0: [f][nr];  chunked = 1: [nr/32][ftotal][32] (CHUNK consecutive grid points per function)
+    int chunked; long fbase; long ftotal;
 };
+constexpr int CHUNK = 32;
+inline long chunked_elems(long nfun, long nr) { return (nr + CHUNK - 1) / CHUNK * CHUNK * nfun; }
 // strided passes along an axis with element stride `stride` over `inner` contiguous elements, `nouter` slabs
 enum SMode { SM_FWD = 0, SM_INV = 1, SM_CONV = 2 /* forward, multiply by ktab, inverse */ };
 struct SArgs {

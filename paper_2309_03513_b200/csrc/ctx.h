@@ -43,6 +43,7 @@ struct tddft_ctx {
     double* d_phi[2] = {nullptr, nullptr};
     double* d_fxc[3] = {nullptr, nullptr, nullptr};
     tddft::cplx* d_work = nullptr;   // [fft_batch][nr]
+    double* d_zeros = nullptr;       // 1 KB of zeros (source of padding rows for the contraction's bulk copies)
     // per-call workspace arena
     char* arena = nullptr; size_t arena_bytes = 0;
     PairTiles tiles[2];

@@ -27,13 +27,20 @@ struct LoadPair {
         return make_double2(re, im);
     }
 };
+struct BatchLayout {     // address of grid point idx of function f inside a batch of real functions (common.h)
+    int chunked; long fbase, cstride, nr;
+    __device__ __forceinline__ long operator()(long f, long idx) const {
+        return chunked ? (idx >> 5) * cstride + (fbase + f) * CHUNK + (idx & (CHUNK - 1)) : (fbase + f) * nr + idx;
+    }
+    __device__ __forceinline__ long next() const { return chunked ? CHUNK : nr; }   // offset from function f to f + 1
+};
 struct LoadPack2 {
-    const double* src0; const double* src1; int nfun; long nr; double scale;
+    const double* src0; const double* src1; int nfun; BatchLayout lay; double scale;
     __device__ __forceinline__ cplx operator()(int b, long idx) const {
-        const long o0 = (long)(2 * b) * nr + idx;
+        const long o0 = lay(2 * b, idx);
         double re = src0[o0]; if (src1) re += src1[o0];
         double im = 0.0;
-        if (2 * b + 1 < nfun) { const long o1 = o0 + nr; im = src0[o1]; if (src1) im += src1[o1]; }
+        if (2 * b + 1 < nfun) { const long o1 = o0 + lay.next(); im = src0[o1]; if (src1) im += src1[o1]; }
         return make_double2(re * scale, im * scale);
     }
 };
@@ -42,11 +49,11 @@ struct StoreWork {
     __device__ __forceinline__ void operator()(int b, long idx, cplx v) const { work[(long)b * nr + idx] = v; }
 };
 struct StoreSplit2 {
-    double* dst; int nfun; long nr; double scale;
+    double* dst; int nfun; BatchLayout lay; double scale;
     __device__ __forceinline__ void operator()(int b, long idx, cplx v) const {
-        const long o0 = (long)(2 * b) * nr + idx;
+        const long o0 = lay(2 * b, idx);
         dst[o0] = v.x * scale;
-        if (2 * b + 1 < nfun) dst[o0 + nr] = v.y * scale;
+        if (2 * b + 1 < nfun) dst[o0 + lay.next()] = v.y * scale;
     }
 };
 
@@ -144,10 +151,10 @@ cudaError_t zpass_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, c
     if (!inverse) {
         // forward passes always store to the work grids
         if (lkind == ZL_PAIR) return zpass_launch<N, false>(LoadPair{a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
-        if (lkind == ZL_PACK2) return zpass_launch<N, false>(LoadPack2{a.src0, a.src1, a.nfun, a.nr, a.lscale}, sw, a, s);
+        if (lkind == ZL_PACK2) return zpass_launch<N, false>(LoadPack2{a.src0, a.src1, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.lscale}, sw, a, s);
         return zpass_launch<N, false>(lw, sw, a, s);
     }
-    if (skind == ZS_SPLIT2) return zpass_launch<N, true>(lw, StoreSplit2{a.dst, a.nfun, a.nr, a.sscale}, a, s);
+    if (skind == ZS_SPLIT2) return zpass_launch<N, true>(lw, StoreSplit2{a.dst, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.sscale}, a, s);
     return zpass_launch<N, true>(lw, sw, a, s);
 }
 template <int N>

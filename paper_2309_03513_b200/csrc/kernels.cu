@@ -62,6 +62,7 @@ cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, c
 }
 
 // ------------------------------------------------------------------------------------------------------
+// a is in the chunked layout [nr/32][nocc*kc][32] (common.h); phi and drho are plain [.][nr]
 template <int KC>
 __global__ void drho_kernel(const double* __restrict__ phi, const double* __restrict__ a, int nocc, int kc, int kk0, long nr,
                             double* __restrict__ drho) {
@@ -70,11 +71,12 @@ __global__ void drho_kernel(const double* __restrict__ phi, const double* __rest
     double acc[KC];
 #pragma unroll
     for (int q = 0; q < KC; ++q) acc[q] = 0.0;
+    const double* ac = a + (r >> 5) * ((long)nocc * kc * CHUNK) + (r & (CHUNK - 1));
     for (int v = 0; v < nocc; ++v) {
         const double p = phi[(long)v * nr + r];
-        const double* av = a + ((long)v * kc + kk0) * nr + r;
+        const double* av = ac + ((long)v * kc + kk0) * CHUNK;
 #pragma unroll
-        for (int q = 0; q < KC; ++q) if (kk0 + q < kc) acc[q] = fma(p, av[(long)q * nr], acc[q]);
+        for (int q = 0; q < KC; ++q) if (kk0 + q < kc) acc[q] = fma(p, av[q * CHUNK], acc[q]);
     }
 #pragma unroll
     for (int q = 0; q < KC; ++q) if (kk0 + q < kc) drho[(long)(kk0 + q) * nr + r] = acc[q];
@@ -102,70 +104,224 @@ cudaError_t launch_hxc_potential(const double* vh, const double* f0, const doubl
 }
 
 __global__ void out_init_kernel(const double* __restrict__ phi, const double* __restrict__ V, const double* __restrict__ vloc,
-                                const double* __restrict__ a, int kc, long nr, double* __restrict__ out) {
-    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (r >= nr) return;
+                                const double* __restrict__ a, int nocc, int kc, long nr, long nrp, double* __restrict__ out) {
+    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;      // r runs over the padded chunks
+    if (r >= nrp) return;
     const int f = blockIdx.y;
     const int v = f / kc, kk = f - v * kc;
+    const long o = (r >> 5) * ((long)nocc * kc * CHUNK) + (long)f * CHUNK + (r & (CHUNK - 1));
     double y = 0.0;
-    if (V) y = phi[(long)v * nr + r] * V[(long)kk * nr + r];
-    if (vloc) y = fma(vloc[r], a[(long)f * nr + r], y);
-    out[(long)f * nr + r] = y;
+    if (r < nr) {
+        if (V) y = phi[(long)v * nr + r] * V[(long)kk * nr + r];
+        if (vloc) y = fma(vloc[r], a[o], y);
+    }
+    out[o] = y;
 }
 cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
                             double* out, cudaStream_t st) {
-    if (!V && !vloc) return cudaMemsetAsync(out, 0, sizeof(double) * nr * nocc * kc, st);
-    dim3 grid((unsigned)((nr + 255) / 256), (unsigned)(nocc * kc));
-    out_init_kernel<<<grid, 256, 0, st>>>(phi, V, vloc, a, kc, nr, out);
+    const long nrp = (nr + CHUNK - 1) / CHUNK * CHUNK;
+    if (!V && !vloc) return cudaMemsetAsync(out, 0, sizeof(double) * nrp * nocc * kc, st);
+    dim3 grid((unsigned)(nrp / 256 + (nrp % 256 ? 1 : 0)), (unsigned)(nocc * kc));
+    out_init_kernel<<<grid, 256, 0, st>>>(phi, V, vloc, a, nocc, kc, nr, nrp, out);
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------------------------------------------
-// S5, first version: one thread per grid point, TI x TK accumulators in registers, FP64 FMA.
-template <int TI, int TK>
-__global__ void __launch_bounds__(128) contract_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau,
-                                const int* __restrict__ slot, int i0, int ti, int j0, int tj, int kc, long nr, double alpha) {
-    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    const int ib = blockIdx.y * TI, kb = blockIdx.z * TK;
-    extern __shared__ int sslot[];     // [TI][tj]
-    for (int t = threadIdx.x; t < TI * tj; t += blockDim.x) {
-        const int i = t / tj, j = t - i * tj;
-        sslot[t] = (ib + i < ti) ? slot[(ib + i) * tj + j] : -1;
-    }
-    __syncthreads();
-    if (r >= nr) return;
-    double acc[TI][TK];
-#pragma unroll
-    for (int i = 0; i < TI; ++i)
-#pragma unroll
-        for (int q = 0; q < TK; ++q) acc[i][q] = 0.0;
-    for (int j = 0; j < tj; ++j) {
-        double av[TK];
-        const double* ap = a + ((long)(j0 + j) * kc + kb) * nr + r;
-#pragma unroll
-        for (int q = 0; q < TK; ++q) av[q] = (kb + q < kc) ? ap[(long)q * nr] : 0.0;
-#pragma unroll
-        for (int i = 0; i < TI; ++i) {
-            const int s = sslot[i * tj + j];
-            const double t = (s >= 0) ? tau[(long)s * nr + r] : 0.0;
-#pragma unroll
-            for (int q = 0; q < TK; ++q) acc[i][q] = fma(t, av[q], acc[i][q]);
+// S5: out[(i0+i)*kc+k][r] -= alpha * sum_j tau_ij(r) a[(j0+j)*kc+k][r]   (Eq. 6).
+// Per grid point this is a (ti x tj)(tj x kc) product whose matrices differ at every r: a batch of N_r small GEMMs,
+// run on the FP64 tensor pipe (mma.sync.m8n8k4.f64).  All real-space batches (tau, a, out) use the chunked layout
+// [nr/32][function][32].  One CTA owns one chunk of 32 grid points, one block of 32 output rows and one direction;
+// its 16 warps take 2 grid points each (32 accumulators per lane).  The operands stream through shared memory in a
+// 4-stage cp.async ring (4 columns per stage: 32 KB of tau + 16 KB of a; every global read is a coalesced 256-byte
+// row; 6 copies of 16 bytes per thread per stage with incrementally updated pointers), rows padded to 272 bytes so
+// that the 16-byte fragment reads are bank-conflict free.  (Bulk async copies were tried: 192 copies of 256 bytes per
+// stage are TMA-issue bound, 2.7x slower.)
+// Off-diagonal tiles use tau twice (out[I] += tau a[J] and out[J] += tau^T a[I]).  The 8 CTAs of a chunk (4 row blocks
+// x 2 directions) are adjacent in launch order and sweep the 4x4 blocks of the tile on a skewed schedule -- direction 1,
+// row block b visits column block (b+t)&3 at step t, direction 2 visits (b-t)&3 -- so both users of a block of tau
+// touch it at about the same time and the second read is an L2 hit: tau crosses HBM about once.
+__device__ __forceinline__ void dmma884k(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int CT_PITCH = CHUNK + 2;                // padded row pitch (doubles): 272 bytes
+constexpr int CT_AROWS = 128;                      // tau rows per stage: 32 rows x 4 columns
+constexpr int CT_STAGES = 4;
+constexpr int CT_WARPS = 16;                       // 2 grid points each
+struct ColSweep {        // the column starts (multiples of 4) a unit visits: blocks of 32 in skewed order, empty blocks skipped
+    int t, cs, cend, wb, dir, ncols;
+    __device__ void settle() {
+        while (t < 4) {
+            const int cb = (dir == 0 ? (wb + t) : (wb - t + 4)) & 3;
+            if (cs < 0) cs = cb * 32;
+            cend = min(cb * 32 + 32, ncols);
+            if (cs < cend) return;
+            ++t; cs = -1;
         }
     }
+    __device__ void init(int dir_, int wb_, int ncols_) { dir = dir_; wb = wb_; ncols = ncols_; t = 0; cs = -1; settle(); }
+    __device__ bool valid() const { return t < 4; }
+    __device__ void next() { cs += 4; if (cs >= cend) { ++t; cs = -1; } settle(); }
+};
+// DUAL = true: off-diagonal tile, dense slots slot(i,j) = i*tj + j, units 0-3 = direction 1, 4-7 = direction 2.
+// DUAL = false: diagonal tile (ti == tj, same orbital block): one direction, tau stored for i <= j only, packed
+// row-major (the order build_tiles emits the pairs), read symmetrically.
+template <int NK, bool DUAL>
+__global__ void __launch_bounds__(32 * CT_WARPS, 1)
+contract_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau, const int* __restrict__ slot,
+                const double* __restrict__ zeros, int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
+    extern __shared__ __align__(16) double sm[];
+    constexpr int BROWS = 4 * 8 * NK;                      // rows of a per stage: 4 columns x (8*NK) trial vectors
+    constexpr int ROWS = CT_AROWS + BROWS;
+    constexpr int STAGE = ROWS * CT_PITCH;                 // doubles
+    constexpr int NCOPY = ROWS / 32;                       // 16-byte copies per thread per stage (512 threads x 16 B = 32 rows)
+    constexpr int NCOPY_A = CT_AROWS / 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long chunk = blockIdx.x >> 3;
+    const int unit = blockIdx.x & 7;
+    const int dir = DUAL ? (unit >> 2) : 0;
+    const int wb = DUAL ? (unit & 3) : (int)(blockIdx.y * 8 + unit);
+    const int nrows = dir == 0 ? ti : tj, ncols = dir == 0 ? tj : ti;
+    const int rowf0 = dir == 0 ? i0 : j0, colf0 = dir == 0 ? j0 : i0;
+    const int rb = wb * 32;
+    if (rb >= nrows) return;
+    const double* tau_c = tau + chunk * stot * CHUNK;
+    const double* a_c = a + chunk * ftot * CHUNK;
+    // this thread's copies: copy q moves piece (tid & 15) of stage row rc = q*32 + (tid >> 4)
+    const int piece2 = (tid & 15) * 2;
+    const int rsub = tid >> 4;                             // 0..31
+    const long a_colstride = (long)kc * CHUNK;             // next column of a
+    // out-of-range rows and columns are zero-filled with plain shared-memory stores (never read from a shared global
+    // zero line: thousands of CTAs hammering one line serialise in L2)
+    auto load_stage = [&](int buf, int cs) {
+        double* base = sm + buf * STAGE;
 #pragma unroll
-    for (int i = 0; i < TI; ++i) {
-        if (ib + i >= ti) continue;
-        double* op = out + ((long)(i0 + ib + i) * kc + kb) * nr + r;
+        for (int q = 0; q < NCOPY; ++q) {
+            const int rc = q * 32 + rsub;
+            const double* src = nullptr;
+            if (q < NCOPY_A) {
+                const int row = rb + (rc >> 2), col = cs + (rc & 3);
+                if (row < nrows && col < ncols) {
+                    long sl;
+                    if (DUAL) sl = dir == 0 ? (long)row * tj + col : (long)col * tj + row;
+                    else {   // diagonal tile: upper triangle packed row-major, slot(i,j) = i(2 tj - i + 1)/2 + (j - i), i <= j
+                        const int lo = min(row, col), hi = max(row, col);
+                        sl = (long)lo * (2 * tj - lo + 1) / 2 + (hi - lo);
+                    }
+                    src = tau_c + sl * CHUNK + piece2;
+                }
+            } else {
+                const int qq = rc - CT_AROWS;
+                const int k = qq >> 2, col = cs + (qq & 3);
+                if (col < ncols && k < kn) src = a_c + (long)(colf0 + col) * a_colstride + (long)k * CHUNK + piece2;
+            }
+            double* dst = base + rc * CT_PITCH + piece2;
+            if (src) cp_async16(dst, src);
+            else *(double2*)dst = make_double2(0.0, 0.0);
+        }
+    };
+    ColSweep issue, use;
+    issue.init(dir, DUAL ? wb : 0, ncols);
+    use = issue;
+    const int lr = lane >> 2, lc = lane & 3;
+    double acc[4][NK][2][2];
 #pragma unroll
-        for (int q = 0; q < TK; ++q) if (kb + q < kc) op[(long)q * nr] = fma(-alpha, acc[i][q], op[(long)q * nr]);
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int n = 0; n < NK; ++n)
+#pragma unroll
+            for (int q = 0; q < 2; ++q) acc[m][n][q][0] = acc[m][n][q][1] = 0.0;
+#pragma unroll
+    for (int st = 0; st < CT_STAGES - 1; ++st) {
+        if (issue.valid()) { load_stage(st, issue.cs); issue.next(); }
+        cp_async_commit();
+    }
+    for (int step = 0; use.valid(); use.next(), ++step) {
+        const int buf = step % CT_STAGES;
+        cp_async_wait<CT_STAGES - 2>();
+        __syncthreads();                                     // stage `step` has landed for every thread; the previous buffer is free
+        if (issue.valid()) { load_stage((step + CT_STAGES - 1) % CT_STAGES, issue.cs); issue.next(); }
+        cp_async_commit();
+        const double* As = sm + buf * STAGE + warp * 2;
+        const double* Bs = As + CT_AROWS * CT_PITCH;
+        double2 af[4], bf[NK];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) af[m] = *(const double2*)(As + ((m * 8 + lr) * 4 + lc) * CT_PITCH);
+#pragma unroll
+        for (int n = 0; n < NK; ++n) bf[n] = *(const double2*)(Bs + ((n * 8 + lr) * 4 + lc) * CT_PITCH);
+#pragma unroll
+        for (int m = 0; m < 4; ++m)
+#pragma unroll
+            for (int n = 0; n < NK; ++n) {
+                dmma884k(acc[m][n][0][0], acc[m][n][0][1], af[m].x, bf[n].x);
+                dmma884k(acc[m][n][1][0], acc[m][n][1][1], af[m].y, bf[n].y);
+            }
+    }
+    cp_async_wait<0>();
+    double* out_c = out + chunk * ftot * CHUNK + warp * 2;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        const int i = rb + m * 8 + lr;
+        if (i >= nrows) continue;
+#pragma unroll
+        for (int n = 0; n < NK; ++n)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int k = n * 8 + 2 * lc + h;
+                if (k >= kn) continue;
+                double2* op = (double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK);
+                double2 x = *op;
+                x.x = fma(-alpha, acc[m][n][0][h], x.x); x.y = fma(-alpha, acc[m][n][1][h], x.y);
+                *op = x;
+            }
     }
 }
-cudaError_t launch_contract(double* out, const double* a, const double* tau, const int* slot, int i0, int ti, int j0, int tj,
-                            int kc, long nr, double alpha, cudaStream_t st) {
-    constexpr int TI = 4, TK = 8;
-    dim3 grid((unsigned)((nr + 127) / 128), (unsigned)((ti + TI - 1) / TI), (unsigned)((kc + TK - 1) / TK));
-    contract_kernel<TI, TK><<<grid, 128, sizeof(int) * TI * tj, st>>>(out, a, tau, slot, i0, ti, j0, tj, kc, nr, alpha);
+
+template <int NK, bool DUAL>
+static cudaError_t contract_launch(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
+                                   int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
+    const size_t smem = sizeof(double) * CT_STAGES * (CT_AROWS + 4 * 8 * NK) * CT_PITCH;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(contract_kernel<NK, DUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    contract_kernel<NK, DUAL><<<grid, 32 * CT_WARPS, smem, st>>>(out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
     return cudaGetLastError();
+}
+cudaError_t launch_contract_single(double* out, const double* a, const double* tau, const int* slot, const double* zeros, int i0, int ti,
+                                   int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st) {
+    const long nchunks = (nr + CHUNK - 1) / CHUNK;
+    dim3 grid((unsigned)(nchunks * 8), (unsigned)((ti + 255) / 256));
+    for (int kb = 0; kb < kc; kb += 16) {
+        const int kn = kc - kb < 16 ? kc - kb : 16;
+        double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
+        cudaError_t e = kn > 8 ? contract_launch<2, false>(grid, o, ap, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
+                               : contract_launch<1, false>(grid, o, ap, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+cudaError_t launch_contract_dual(double* out, const double* a, const double* tau, const double* zeros, int i0, int ti, int j0, int tj,
+                                 int kc, long ftot, long nr, double alpha, cudaStream_t st) {
+    if (ti > 128 || tj > 128) return cudaErrorInvalidValue;
+    const long nchunks = (nr + CHUNK - 1) / CHUNK;
+    dim3 grid((unsigned)(nchunks * 8));
+    for (int kb = 0; kb < kc; kb += 16) {
+        const int kn = kc - kb < 16 ? kc - kb : 16;
+        double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
+        cudaError_t e = kn > 8 ? contract_launch<2, true>(grid, o, ap, tau, nullptr, zeros, i0, ti, j0, tj, kc, kn, ftot, (long)ti * tj, alpha, st)
+                               : contract_launch<1, true>(grid, o, ap, tau, nullptr, zeros, i0, ti, j0, tj, kc, kn, ftot, (long)ti * tj, alpha, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------------

@@ -1,7 +1,7 @@
 // Launch wrappers of the non-FFT kernels (kernels.cu, gemm.cu).  All asynchronous on the given stream.
 #pragma once
 #include <cuda_runtime.h>
-#include "fft_core.cuh"
+#include "common.h"
 
 namespace tddft {
 
@@ -28,9 +28,14 @@ cudaError_t launch_hxc_potential(const double* vh, const double* f0, const doubl
 // S5 start value: out[f][r] = phi[v][r]*V[kk][r] (if V) + vloc[r]*a[f][r] (if vloc), f = v*kc+kk
 cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
                             double* out, cudaStream_t st);
-// S5: out[(i0+i)*kc+kk][r] -= alpha * sum_{j<tj} tau[slot[i*tj+j]][r] * a[(j0+j)*kc+kk][r]   (Eq. 6)
-cudaError_t launch_contract(double* out, const double* a, const double* tau, const int* slot, int i0, int ti, int j0, int tj,
-                            int kc, long nr, double alpha, cudaStream_t st);
+// S5 (Eq. 6) on batches in the chunked layout [nr/32][function][32] (common.h); ftot = functions in
+// a/out (nocc*kc), stot = slots in the tau tile.
+// single: out[(i0+i)*kc+k] -= alpha sum_{j<tj} tau[slot[i*tj+j]] a[(j0+j)*kc+k]    (diagonal tiles; slot table on device)
+// dual:   that with slot(i,j) = i*tj+j AND out[(j0+j)*kc+k] -= alpha sum_i tau[i*tj+j] a[(i0+i)*kc+k]   (off-diagonal tiles)
+cudaError_t launch_contract_single(double* out, const double* a, const double* tau, const int* slot, const double* zeros, int i0, int ti,
+                                   int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st);
+cudaError_t launch_contract_dual(double* out, const double* a, const double* tau, const double* zeros, int i0, int ti, int j0, int tj,
+                                 int kc, long ftot, long nr, double alpha, cudaStream_t st);   // zeros: 256 B of device zeros
 // S0: rho[r] = sum_v phi[v][r]^2 ; LDA kernel f_xc (Eq. 8; reading A5)
 cudaError_t launch_rho0(const double* phi, int nocc, long nr, double* rho, cudaStream_t st);
 cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double* fuu, double* fud,

@@ -73,6 +73,7 @@ typedef struct {
   const double* x0;         /* device, n_x0 start vectors in the mode's layout, or NULL: library draws its own */
   int n_x0;
   unsigned long long seed;  /* seed of the library's own start vectors */
+  int fft_path;             /* 0 = fused plane/x kernels when the grid shape has them (default), 1 = general pass kernels only */
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,

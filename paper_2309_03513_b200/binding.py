@@ -29,7 +29,7 @@ class tddft_options(C.Structure):
         ("vloc_up", C.c_void_p), ("vloc_dn", C.c_void_p), ("cuda_stream", C.c_void_p),
         ("workspace_gb", C.c_double), ("pair_tile", C.c_int), ("fft_batch", C.c_int),
         ("max_subspace", C.c_int), ("max_iter", C.c_int), ("tol", C.c_double),
-        ("x0", C.c_void_p), ("n_x0", C.c_int), ("seed", C.c_ulonglong),
+        ("x0", C.c_void_p), ("n_x0", C.c_int), ("seed", C.c_ulonglong), ("fft_path", C.c_int),
     ]
 
 

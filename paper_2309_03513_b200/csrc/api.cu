@@ -79,10 +79,35 @@ static SArgs xpass_args(const tddft_ctx* c, int batch) {
 }
 static ZArgs zpass_args(const tddft_ctx* c, int batch) {
     const int* n = c->hp.n;
-    ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.work = c->d_work;
+    ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.tw2 = c->d_tw[1]; a.work = c->d_work;
     a.lscale = 1.0; a.sscale = 1.0;
     return a;
 }
+
+// The three legs of every transform: (y,z) forward with a fused load, the x pass (forward / inverse / forward *
+// Coulomb table * inverse), (y,z) inverse with a fused split store.  Fused plane/x kernels when the grid shape has
+// them (fft_fused.cu), otherwise one general pass kernel per axis.
+static int leg_forward_yz(tddft_ctx* c, int lkind, const ZArgs& z) {
+    if (c->fused) { TD_CUDA(c, launch_plane(c->hp.n[1], c->hp.n[2], false, lkind, ZS_WORK, z, c->stream)); c->stats.kernel_launches += 1; return TDDFT_OK; }
+    TD_CUDA(c, launch_zpass(false, lkind, ZS_WORK, z, c->stream));
+    TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, z.batch), c->stream));
+    c->stats.kernel_launches += 2;
+    return TDDFT_OK;
+}
+static int leg_x(tddft_ctx* c, int mode, int nb) {
+    if (c->fused) TD_CUDA(c, launch_xpass(mode, xpass_args(c, nb), c->stream));
+    else TD_CUDA(c, launch_spass(mode, xpass_args(c, nb), c->stream));
+    c->stats.kernel_launches += 1;
+    return TDDFT_OK;
+}
+static int leg_inverse_yz(tddft_ctx* c, const ZArgs& z) {
+    if (c->fused) { TD_CUDA(c, launch_plane(c->hp.n[1], c->hp.n[2], true, ZL_WORK, ZS_SPLIT2, z, c->stream)); c->stats.kernel_launches += 1; return TDDFT_OK; }
+    TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, z.batch), c->stream));
+    TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
+    c->stats.kernel_launches += 2;
+    return TDDFT_OK;
+}
+#define TD_RC(call) do { int rc_ = (call); if (rc_) return rc_; } while (0)
 
 // tau_p = C[phi_i phi_j] for npairs pairs (device list), two pairs per complex grid
 static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, long npairs, double* tau, int chunked) {
@@ -92,13 +117,10 @@ static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pa
         const int nb = (np + 1) / 2;
         ZArgs z = zpass_args(c, nb);
         z.phi = phi; z.pairs = d_pairs + p0; z.npairs = np;
-        TD_CUDA(c, launch_zpass(false, ZL_PAIR, ZS_WORK, z, c->stream));
-        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        TD_RC(leg_forward_yz(c, ZL_PAIR, z));
+        TD_RC(leg_x(c, SM_CONV, nb));
         z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = p0; z.ftotal = npairs;
-        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
-        c->stats.kernel_launches += 5;
+        TD_RC(leg_inverse_yz(c, z));
         c->stats.pair_ffts += np;
     }
     return TDDFT_OK;
@@ -112,12 +134,11 @@ static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, d
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
         const int nb = (nf + 1) / 2;
         TD_CUDA(c, launch_scatter_pack2(X, lay, f0, nfun, nb, c->d_idx_p, c->d_idx_m, c->d_work, nr, c->stream));
-        TD_CUDA(c, launch_spass(SM_INV, xpass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        TD_RC(leg_x(c, SM_INV, nb));
         ZArgs z = zpass_args(c, nb);
         z.dst = dst; z.nfun = nf; z.sscale = scale; z.chunked = chunked; z.fbase = f0; z.ftotal = nfun;
-        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
-        c->stats.kernel_launches += 4;
+        TD_RC(leg_inverse_yz(c, z));
+        c->stats.kernel_launches += 1;
     }
     return TDDFT_OK;
 }
@@ -131,11 +152,10 @@ static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cpl
         const int nb = (nf + 1) / 2;
         ZArgs z = zpass_args(c, nb);
         z.src0 = src; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0; z.chunked = 1; z.fbase = f0; z.ftotal = nfun;
-        TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
-        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_FWD, xpass_args(c, nb), c->stream));
+        TD_RC(leg_forward_yz(c, ZL_PACK2, z));
+        TD_RC(leg_x(c, SM_FWD, nb));
         TD_CUDA(c, launch_gather_unpack2(c->d_work, nr, c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream));
-        c->stats.kernel_launches += 4;
+        c->stats.kernel_launches += 1;
     }
     return TDDFT_OK;
 }
@@ -148,25 +168,40 @@ static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scal
         const int nb = (nf + 1) / 2;
         ZArgs z = zpass_args(c, nb);
         z.src0 = d0; z.src1 = d1; z.nfun = nf; z.lscale = scale; z.chunked = 0; z.fbase = f0; z.ftotal = kc;
-        TD_CUDA(c, launch_zpass(false, ZL_PACK2, ZS_WORK, z, c->stream));
-        TD_CUDA(c, launch_spass(SM_FWD, ypass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_CONV, xpass_args(c, nb), c->stream));
-        TD_CUDA(c, launch_spass(SM_INV, ypass_args(c, nb), c->stream));
+        TD_RC(leg_forward_yz(c, ZL_PACK2, z));
+        TD_RC(leg_x(c, SM_CONV, nb));
         z.dst = vh; z.sscale = 1.0;
-        TD_CUDA(c, launch_zpass(true, ZL_WORK, ZS_SPLIT2, z, c->stream));
-        c->stats.kernel_launches += 5;
+        TD_RC(leg_inverse_yz(c, z));
     }
     return TDDFT_OK;
 }
 
 // S8: rows <- P_c rows with the occupied orbitals of tgt_spin, two tensor-core GEMMs
-int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_stride, double* O) {
+int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_stride, double* O, size_t o_cap) {
     const long k2 = 2 * c->hp.npwh;
     const int no = c->nocc[tgt];
-    TD_CUDA(c, launch_gemm_nt(c->psi[tgt], k2, Y, k2, grp, grp_stride, O, nrows, no, nrows, k2, k2, 2.0, 1, nullptr, c->stream));
-    TD_CUDA(c, launch_gemm_tn_acc(O, nrows, c->psi[tgt], k2, Y, k2, grp, grp_stride, nrows, k2, no, -1.0, c->stream));
-    c->stats.kernel_launches += 2;
+    const long ldo = (nrows + 1) & ~1L;                      // even pitch: 16-byte aligned rows for the async copies
+    // k splits chosen so that the CTAs fill whole waves of the SMs (ordered reduction, deterministic)
+    const long tiles = gemm_nt_tile_count(no, nrows);
+    int splits = 1; double best = 0.0;
+    for (int s = 1; s <= 16; ++s) {
+        if ((size_t)no * ldo + (size_t)s * no * nrows > o_cap || k2 / s < 256) break;
+        const long ctas = tiles * s, waves = (ctas + c->num_sms - 1) / c->num_sms;
+        const double eff = (double)ctas / (double)(waves * c->num_sms);
+        if (eff > best + 0.02) { best = eff; splits = s; }
+    }
+    double* partial = splits > 1 ? O + (size_t)no * ldo : nullptr;
+    TD_CUDA(c, launch_gemm_nt(c->psi[tgt], k2, Y, k2, grp, grp_stride, O, ldo, no, nrows, k2, k2, 2.0, splits, partial, c->stream));
+    TD_CUDA(c, launch_gemm_tn_acc(O, ldo, c->psi[tgt], k2, Y, k2, grp, grp_stride, nrows, k2, no, -1.0, c->stream));
+    c->stats.kernel_launches += 2 + (splits > 1 ? 1 : 0);
     return TDDFT_OK;
+}
+size_t project_scratch_doubles(const tddft_ctx* c, int maxocc, int nrows, size_t max_bytes) {
+    const size_t one = (size_t)maxocc * ((nrows + 1) & ~1L);
+    size_t cap = std::min<size_t>((size_t)1 << 28, max_bytes / 8 / sizeof(double));   // k-split partial sums: <= 2 GB and <= 1/8 of the budget
+    int mult = 13;
+    while (mult > 1 && one * mult > cap) --mult;
+    return one * mult;
 }
 
 // ---- pair tiles -------------------------------------------------------------------------------------
@@ -244,7 +279,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
     for (;;) {
         fixed = grid_b * (size_t)kc * ((size_t)sumocc + (size_t)maxocc + (hxc ? 2 * blocks.size() + 1 : 0))
-              + sizeof(double) * (size_t)maxocc * (size_t)kc * (size_t)maxocc + 4096;
+              + sizeof(double) * project_scratch_doubles(c, maxocc, kc * maxocc, budget) + 4096;
         T = std::min(std::min(maxocc, 128), c->pair_tile > 0 ? c->pair_tile : 128);
         const int tmin = std::min(maxocc, 16);
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 8);
@@ -263,7 +298,8 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     std::vector<double*> drho(blocks.size(), nullptr), V(blocks.size(), nullptr);
     double* vh = nullptr;
     if (hxc) { for (size_t b = 0; b < blocks.size(); ++b) { drho[b] = carve(grid_b * kc); V[b] = carve(grid_b * kc); } vh = carve(grid_b * kc); }
-    double* O = carve(sizeof(double) * (size_t)maxocc * kc * maxocc);
+    const size_t o_cap = project_scratch_doubles(c, maxocc, kc * maxocc, budget);
+    double* O = carve(sizeof(double) * o_cap);
     double* tau = carve(grid_b * (size_t)T * T);
     for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src])); if (rc) return rc; }
 
@@ -312,7 +348,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
             { StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, X, AX, lay, c->d_eig[bl.src]); if (rc) return rc; }
             // S8: conduction-band projector of the target spin
             { StageTimer t(c, ST_S8);
-              rc = project_rows(c, bl.tgt, (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, O); if (rc) return rc; }
+              rc = project_rows(c, bl.tgt, (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, O, o_cap); if (rc) return rc; }
         }
     }
     collect_timing(c);
@@ -371,6 +407,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         const char* perr = build_host_plan(lattice, grid, ecut, &c->hp);
         if (perr) return fail(std::strstr(perr, "plan") ? TDDFT_EUNSUPPORTED : TDDFT_EINVAL, std::string("init: ") + perr);
         c->ecut = ecut; c->alpha = alpha; c->nspin = nspin;
+        { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev); if (c->num_sms < 1) c->num_sms = 148; }
         c->nocc[0] = nocc[0]; c->nocc[1] = nspin == 2 ? nocc[1] : 0;
         c->psi[0] = psi_up; c->psi[1] = nspin == 2 ? psi_dn : nullptr;
         c->eig_h[0].assign(eig_up, eig_up + nocc[0]);
@@ -384,7 +421,9 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->workspace_gb = opt->workspace_gb; c->pair_tile = opt->pair_tile; c->fft_batch = opt->fft_batch;
             c->dav_max_subspace = opt->max_subspace; c->dav_max_iter = opt->max_iter; c->dav_tol = opt->tol;
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
-        }
+            c->fused = opt->fft_path == 0;
+        } else c->fused = true;
+        c->fused = c->fused && fused_supported(grid);
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) c->fft_batch = (int)std::max<long>(1, std::min<long>(64, (64L << 20) / (16 * nr)));
 #define INIT_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? TDDFT_ENOMEM : TDDFT_ECUDA, std::string("init: " #call ": ") + cudaGetErrorString(e_)); } while (0)
@@ -492,9 +531,10 @@ int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs
 
 int tddft_project(tddft_ctx* c, int spin, double* Y, long nfun) {
     if (!c || !Y || nfun < 1 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
-    int rc = ensure_arena(c, sizeof(double) * (size_t)c->nocc[spin] * nfun);
+    const size_t cap = project_scratch_doubles(c, c->nocc[spin], (int)nfun, (size_t)1 << 34);
+    int rc = ensure_arena(c, sizeof(double) * cap);
     if (rc) return rc;
-    return project_rows(c, spin, Y, (int)nfun, (int)nfun, 0, (double*)c->arena);
+    return project_rows(c, spin, Y, (int)nfun, (int)nfun, 0, (double*)c->arena, cap);
 }
 
 int tddft_gram(tddft_ctx* c, const double* V, const double* W, int m, long n_complex, double* G) {

@@ -19,6 +19,7 @@ struct ZArgs {
     long nr;               // points per grid
     int batch;             // packed grids in this launch
     const cplx* tw;        // device twiddles exp(-2 pi i k/n)
+    const cplx* tw2;       // fused plane kernels only: twiddles of the y axis
     cplx* work;            // [batch][nr] complex work grids (source for ZL_WORK, destination for ZS_WORK)
     // ZL_PAIR: packed grid b = phi[pairs[2b].x]*phi[pairs[2b].y] + i phi[pairs[2b+1].x]*phi[pairs[2b+1].y]
     const double* phi;     // [norb][nr]
@@ -48,5 +49,9 @@ bool fft_size_supported(int n);
 cudaError_t launch_zpass(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st);
 cudaError_t launch_spass(int mode, const SArgs& a, cudaStream_t st);
 void fft_plan_radices(int n, int* r1, int* r2, int* r3);   // 0s if unsupported
+// fused fast path (fft_fused.cu): y+z transforms of one x-plane per CTA, register-resident x pass
+bool fused_supported(const int* n);
+cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st);
+cudaError_t launch_xpass(int mode, const SArgs& a, cudaStream_t st);
 
 }  // namespace tddft

@@ -34,6 +34,8 @@ struct tddft_ctx {
     cudaStream_t stream = nullptr;
     double workspace_gb = 0;
     int pair_tile = 0, fft_batch = 0;
+    int num_sms = 148;
+    bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off
     int dav_max_subspace = 0, dav_max_iter = 0; double dav_tol = 0; const double* dav_x0 = nullptr; int dav_nx0 = 0;
     unsigned long long seed = 0;
     // device tables
@@ -59,7 +61,8 @@ int set_err(tddft_ctx* c, int status, const std::string& msg);
 int apply_liouville_dev(tddft_ctx* c, const double* X, double* AX, int nvec, int mode);
 long vector_len(const tddft_ctx* c, int mode);
 // P_c on functions laid out as rows: row n at Y + (n / grp)*grp_stride + (n % grp)*2*npwh (doubles); scratch O from arena
-int project_rows(tddft_ctx* c, int tgt_spin, double* Y, int nrows, int grp, long grp_stride, double* O);
+int project_rows(tddft_ctx* c, int tgt_spin, double* Y, int nrows, int grp, long grp_stride, double* O, size_t o_cap);
+size_t project_scratch_doubles(const tddft_ctx* c, int maxocc, int nrows, size_t max_bytes);   // capacity (doubles) project_rows wants for O
 int ensure_arena(tddft_ctx* c, size_t bytes);
 }  // namespace tddft
 

@@ -172,7 +172,8 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     DV_TRY(cudaMalloc((void**)&XR, sizeof(double) * n2 * 3 * nroots));     // X (Ritz), R (residual / W-combination), WY for restarts
     DV_TRY(cudaMalloc((void**)&T, sizeof(double) * n2));
     DV_TRY(cudaMalloc((void**)&small, sizeof(double) * small_n));
-    DV_TRY(cudaMalloc((void**)&Oproj, sizeof(double) * (size_t)maxocc * maxocc));
+    const size_t oproj_cap = project_scratch_doubles(c, maxocc, maxocc, (size_t)1 << 34);
+    DV_TRY(cudaMalloc((void**)&Oproj, sizeof(double) * oproj_cap));
     double* X = XR; double* R = XR + n2 * nroots; double* WY = XR + 2 * n2 * nroots;
     double* H = small; double* Hwork = H + (size_t)max_sub * max_sub; double* Y = Hwork + (size_t)max_sub * max_sub;
     double* part = Y + (size_t)max_sub * max_sub; double* theta = part + (size_t)max_sub * max_sub * splits;
@@ -183,7 +184,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
 
     auto project_vec = [&](double* x) -> int {     // P_c block by block on one full vector
         for (auto& b : blocks) {
-            int rc = project_rows(c, b.tgt, x + 2 * b.off, c->nocc[b.src], c->nocc[b.src], 0, Oproj);
+            int rc = project_rows(c, b.tgt, x + 2 * b.off, c->nocc[b.src], c->nocc[b.src], 0, Oproj, oproj_cap);
             if (rc) return rc;
         }
         return TDDFT_OK;

@@ -1,0 +1,83 @@
+// Instantiations and host dispatch of the fused FFT kernels (fft_fused.cuh) for the grid shapes of the BASELINE.json
+// configurations that fit the fast path; every other shape runs the general pass kernels (fft_steps.cuh).
+#include "fft_fused.cuh"
+
+namespace tddft {
+
+// (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
+#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8)
+#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
+
+template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
+static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
+    static_assert(Two<NY>::ok && Two<NZ>::ok, "fused plane kernel needs two-stage plans");
+    const size_t smem = sizeof(cplx) * (size_t)NY * Two<NZ>::PITCH;
+    auto kern = plane_kernel<NY, NZ, NTHR, MINB, INV, Load, Store>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid((unsigned)(a.npencils / NY), (unsigned)a.batch);
+    kern<<<grid, NTHR, smem, s>>>(ld, st, a.tw2, a.tw);
+    return cudaGetLastError();
+}
+template <int NY, int NZ, int NTHR, int MINB>
+static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
+    LoadWork lw{a.work, a.nr};
+    StoreWork sw{a.work, a.nr};
+    const BatchLayout lay{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr};
+    if (!inverse) {
+        if (lkind == ZL_PAIR) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
+        if (lkind == ZL_PACK2) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPack2{a.src0, a.src1, a.nfun, lay, a.lscale}, sw, a, s);
+        return cudaErrorInvalidValue;
+    }
+    if (skind == ZS_SPLIT2) return plane_launch<NY, NZ, NTHR, MINB, true>(lw, StoreSplit2{a.dst, a.nfun, lay, a.sscale}, a, s);
+    return cudaErrorInvalidValue;
+}
+
+template <int NX>
+static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
+    static_assert(Two<NX>::ok, "fused x pass needs a two-stage plan");
+    constexpr size_t smem = XCfg<NX>::SMEM;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(xpass_kernel<NX, SM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_CONV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid((unsigned)((a.inner + XW - 1) / XW), (unsigned)a.batch);
+    constexpr int NT = XCfg<NX>::NTHR;
+    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab);
+    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab);
+    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab);
+    return cudaGetLastError();
+}
+
+bool fused_supported(const int* n) {
+    bool px = false, pl = false;
+#define X(N) if (n[0] == N) px = true;
+    TD_FOR_EACH_XLEN(X)
+#undef X
+#define X(NY, NZ, T, B) if (n[1] == NY && n[2] == NZ) pl = true;
+    TD_FOR_EACH_PLANE(X)
+#undef X
+    return px && pl;
+}
+cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st) {
+#define X(NY, NZ, T, B) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B>(inverse, lkind, skind, a, st);
+    TD_FOR_EACH_PLANE(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+cudaError_t launch_xpass(int mode, const SArgs& a, cudaStream_t st) {
+#define X(N) if (a.n == N) return xpass_launch<N>(mode, a, st);
+    TD_FOR_EACH_XLEN(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace tddft

@@ -3,6 +3,7 @@
 // tcgen05 has no FP64 path, so the FP64 tensor pipe is reached through mma.sync; measured DMMA peak on B200 equals
 // the DFMA peak (36.9 TFLOP/s), the gain is issue slots and register traffic, not raw rate.
 #include "kernels.h"
+#include "gemm_pipe.cuh"
 
 namespace tddft {
 
@@ -84,13 +85,44 @@ __global__ void splitk_reduce_kernel(const double* __restrict__ partial, int spl
     for (int z = 0; z < splits; ++z) s += partial[(long)z * mn + i];
     C[(i / N) * ldc + (i % N)] = cscale * s;
 }
+template <class CFG>
+static cudaError_t nt_pipe_launch(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
+                                  int M, int N, long K, long kper, long wperiod, double cscale, int splits, double* partial, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_nt_pipe_kernel<CFG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM_NT);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid((unsigned)((N + CFG::BN - 1) / CFG::BN), (unsigned)((M + CFG::BM - 1) / CFG::BM), (unsigned)splits);
+    gemm_nt_pipe_kernel<CFG><<<grid, CFG::NTHR, CFG::SMEM_NT, st>>>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial);
+    return cudaGetLastError();
+}
+typedef GemmCfg<144, 128, 72, 32, 4> NtBig;     // orbitals x functions: 432 = 3 x 144, 1150 ~ 8 x 144
+typedef GemmCfg<64, 64, 32, 32, 4> NtSmall;     // Davidson Gram matrices (m <= a few hundred, K = 10^7)
+typedef GemmCfg<128, 144, 32, 72, 4> TnBig;
+
+int gemm_nt_tile_count(int M, int N) {
+    if (M >= 96 && N >= 96) return ((M + NtBig::BM - 1) / NtBig::BM) * ((N + NtBig::BN - 1) / NtBig::BN);
+    return ((M + 63) / 64) * ((N + 63) / 64);
+}
 cudaError_t launch_gemm_nt(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
                            int M, int N, long K, long wperiod, double cscale, int splits, double* partial, cudaStream_t st) {
     if (splits < 1 || !partial) splits = 1;
     long kper = ((K + splits - 1) / splits + BK - 1) / BK * BK;
     splits = (int)((K + kper - 1) / kper);
-    dim3 grid((unsigned)((N + BN - 1) / BN), (unsigned)((M + BM - 1) / BM), (unsigned)splits);
-    gemm_nt_kernel<<<grid, 128, 0, st>>>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial);
+    const bool aligned = (lda % 2 == 0) && (ldb % 2 == 0) && (bstride_grp % 2 == 0) && (((size_t)A | (size_t)B) % 16 == 0);
+    cudaError_t e;
+    if (!aligned) {
+        dim3 grid((unsigned)((N + BN - 1) / BN), (unsigned)((M + BM - 1) / BM), (unsigned)splits);
+        gemm_nt_kernel<<<grid, 128, 0, st>>>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial);
+        e = cudaGetLastError();
+    } else if (M >= 96 && N >= 96) {
+        e = nt_pipe_launch<NtBig>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial, st);
+    } else {
+        e = nt_pipe_launch<NtSmall>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial, st);
+    }
+    if (e != cudaSuccess) return e;
     if (splits > 1) {
         const long mn = (long)M * N;
         splitk_reduce_kernel<<<(unsigned)((mn + 255) / 256), 256, 0, st>>>(partial, splits, mn, N, C, ldc, cscale);
@@ -140,6 +172,18 @@ __global__ void __launch_bounds__(128) gemm_tn_acc_kernel(const double* __restri
 }
 cudaError_t launch_gemm_tn_acc(const double* At, long ldat, const double* B, long ldb, double* C, long ldc, int cgrp,
                                long cstride_grp, int M, long N, int K, double cscale, cudaStream_t st) {
+    const bool aligned = (ldat % 2 == 0) && (ldb % 2 == 0) && (((size_t)At | (size_t)B) % 16 == 0);
+    if (aligned && M >= 96 && N >= 96) {
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaError_t e = cudaFuncSetAttribute(gemm_tn_pipe_kernel<TnBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TnBig::SMEM_TN);
+            if (e != cudaSuccess) return e;
+            attr_done = true;
+        }
+        dim3 grid((unsigned)((N + TnBig::BN - 1) / TnBig::BN), (unsigned)((M + TnBig::BM - 1) / TnBig::BM));
+        gemm_tn_pipe_kernel<TnBig><<<grid, TnBig::NTHR, TnBig::SMEM_TN, st>>>(At, ldat, B, ldb, C, ldc, cgrp, cstride_grp, M, N, K, cscale);
+        return cudaGetLastError();
+    }
     dim3 grid((unsigned)((N + BN - 1) / BN), (unsigned)((M + BM - 1) / BM));
     gemm_tn_acc_kernel<<<grid, 128, 0, st>>>(At, ldat, B, ldb, C, ldc, cgrp, cstride_grp, M, N, K, cscale);
     return cudaGetLastError();

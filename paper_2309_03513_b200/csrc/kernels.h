@@ -47,6 +47,7 @@ cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, 
 // K may be split over `splits` CTAs along k; partial sums go to `partial` [splits][m][n] and are reduced in order.
 cudaError_t launch_gemm_nt(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
                            int M, int N, long K, long wperiod, double cscale, int splits, double* partial, cudaStream_t st);
+int gemm_nt_tile_count(int M, int N);   // CTAs per k split of launch_gemm_nt (for choosing splits that fill the SMs)
 // C[m][n] += cscale * sum_k At[k][m] B[k][n];  C row m at  C + (m / cgrp)*cstride_grp + (m % cgrp)*ldc
 cudaError_t launch_gemm_tn_acc(const double* At, long ldat, const double* B, long ldb, double* C, long ldc, int cgrp,
                                long cstride_grp, int M, long N, int K, double cscale, cudaStream_t st);

@@ -1,0 +1,99 @@
+"""GPU parity at the BASELINE.json sizes, in the launch configuration bench.py times (reading A19).
+
+The oracle needs N_occ pair potentials per output column, so at configs 2 and 3 it computes a seeded sample of the
+columns (spin, v, k) of AX one by one (`Problem.column`); the full GPU result is checked against the invariants that
+hold at any size: symmetry <Y|AX> = <AY|X> and P_c AX = AX.  Tolerance 1e-10 relative (north star), FP64.
+"""
+import numpy as np
+import pytest
+
+from helpers import Case, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+TRI = [[7.0, 0, 0], [0.9, 7.4, 0], [0.5, -0.4, 6.6]]
+
+
+def _sampled_columns(case, X, got, mode, samples):
+    o = case.oracle
+    L = o.vector_len(mode)
+    got = got.reshape(X.shape[0], L)
+    off = [0]
+    if mode == 0:
+        for s in range(o.nspin - 1):
+            off.append(off[-1] + o.nocc[s] * o.npwh)
+    worst = 0.0
+    for k in sorted({k for k, _, _ in samples}):
+        ctx = o.prepare(X[k], mode)
+        for kk, s, v in samples:
+            if kk != k:
+                continue
+            ref = o.column(ctx, s, v)
+            a = off[s] + v * o.npwh
+            worst = max(worst, rel_fro(got[k, a:a + o.npwh], ref))
+    return worst
+
+
+def _invariants(case, X, got, mode):
+    o = case.oracle
+    n = X.shape[0]
+    M = np.array([[o.vdot(X[i], got[j]) for j in range(n)] for i in range(n)])
+    assert np.max(np.abs(M - M.T)) < 1e-11 * np.max(np.abs(M)), "A is not symmetric on the GPU result"
+    for k in (0, n - 1):
+        p = o.project_vector(got[k], mode)
+        assert rel_fro(p, got[k].reshape(-1)) < 1e-12, "P_c AX != AX"
+
+
+@pytest.mark.parametrize("fft_path", [0, 1])
+def test_pair_potentials_fused_and_general_paths(fft_path):
+    # (12,18,20): radices 3,4 / 3,6 / 5,4 -- a shape with fused plane and x kernels, NY != NZ, ragged x tiles
+    import torch
+    from paper_2309_03513_b200 import binding as b
+    case = Case(TRI, (12, 18, 20), 6.0, 2, (5, 4), 0.3, seed=201, fft_path=fft_path, fft_batch=2)
+    ctx = case.ctx()
+    nr = int(np.prod(case.grid))
+    pairs = [(i, j) for i in range(5) for j in range(i, 5)]
+    tau = torch.empty((len(pairs), nr), dtype=torch.float64, device="cuda")
+    b.tddft_pair_potentials(ctx, 0, pairs, tau)
+    tau = tau.cpu().numpy()
+    for p, (i, j) in enumerate(pairs):
+        ref = case.oracle.coulomb(case.oracle.phi[0][i] * case.oracle.phi[0][j]).reshape(-1)
+        assert rel_fro(tau[p], ref) < 1e-12
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_apply_fused_shape_triclinic(mode):
+    case = Case(TRI, (12, 18, 20), 6.0, 2, (5, 4), 0.3, seed=202, vloc=True)
+    X = case.trial(3, mode)
+    assert rel_fro(case.gpu_apply(X, mode), case.oracle.apply(X, mode)) < TOL
+
+
+def test_apply_config1_general_path_equals_fused():
+    fused = Case.from_config(1)
+    X = fused.trial(4, 0)
+    ref = fused.oracle.apply(X, 0)
+    assert rel_fro(fused.gpu_apply(X, 0), ref) < TOL
+    general = Case.from_config(1, oracle=False, fft_path=1)
+    assert rel_fro(general.gpu_apply(X, 0), ref) < TOL
+
+
+def test_apply_config2_sampled_columns():
+    # BASELINE.json configs[1]: 48^3, 129/127 orbitals, 8 trial vectors, alpha = 0.18
+    case = Case.from_config(2)
+    X = case.trial(8, 0)
+    got = case.gpu_apply(X, 0)
+    samples = [(0, 0, 0), (0, 0, 128), (0, 1, 63), (5, 0, 77), (5, 1, 126), (7, 1, 0)]
+    assert _sampled_columns(case, X, got, 0, samples) < TOL
+    _invariants(case, X, got, 0)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_apply_config3_sampled_columns(mode):
+    # BASELINE.json configs[2], the bench workload: 72^3, 432/430 orbitals, 16 trial vectors, both modes
+    case = Case.from_config(3, fft_backend="numpy")   # library FFT as the oracle's transform step (pinned equal to the radix FFT)
+    X = case.trial(16, mode)
+    got = case.gpu_apply(X, mode)
+    samples = [(3, 0, 431), (3, 1, 17)] if mode == 0 else [(11, 0, 200)]
+    assert _sampled_columns(case, X, got, mode, samples) < TOL
+    _invariants(case, X, got, mode)

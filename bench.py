@@ -274,7 +274,7 @@ def main():
     peak, peak_src = measured_peaks()
     s4_ms = stage_ms.get("ms_s4_pair_fft", 0.0)
     pairs_per_step = pair_ffts / max(args.steps, 1)
-    fft_batch = args.fft_batch or max(1, min(64, (64 << 20) // (16 * nr)))
+    fft_batch = args.fft_batch or max(1, min(64, (192 << 20) // (16 * nr)))
     roofline = None
     if s4_ms > 0 and pair_ffts > 0:
         bytes_per_pair = 32.0 * nr                      # one HBM round trip per direction per pair density

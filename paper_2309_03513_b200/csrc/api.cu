@@ -425,7 +425,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         } else c->fused = true;
         c->fused = c->fused && fused_supported(grid);
         const long nr = c->hp.nr, npwh = c->hp.npwh;
-        if (c->fft_batch <= 0) c->fft_batch = (int)std::max<long>(1, std::min<long>(64, (64L << 20) / (16 * nr)));
+        if (c->fft_batch <= 0) c->fft_batch = (int)std::max<long>(1, std::min<long>(64, (192L << 20) / (16 * nr)));   // latency-bound kernels: large launches beat L2 residency (measured)
 #define INIT_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? TDDFT_ENOMEM : TDDFT_ECUDA, std::string("init: " #call ": ") + cudaGetErrorString(e_)); } while (0)
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_p, sizeof(int) * npwh));
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_m, sizeof(int) * npwh));

@@ -1,5 +1,6 @@
 // Instantiations and host dispatch of the fused FFT kernels (fft_fused.cuh) for the grid shapes of the BASELINE.json
 // configurations that fit the fast path; every other shape runs the general pass kernels (fft_steps.cuh).
+#include <cstdlib>
 #include "fft_fused.cuh"
 
 namespace tddft {
@@ -8,20 +9,47 @@ namespace tddft {
 #define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8)
 #define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
 
-template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
-static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
+static int plane_variant() {          // experiment switch: bit0 persistent grid, bit1 DB1, bit2 DB2, bit3 L2 prefetch
+    static int v = -1;
+    if (v < 0) { const char* e = getenv("TDDFT_VAR"); v = e ? atoi(e) : 9; }
+    return v;
+}
+template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
+static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
     static_assert(Two<NY>::ok && Two<NZ>::ok, "fused plane kernel needs two-stage plans");
     const size_t smem = sizeof(cplx) * (size_t)NY * Two<NZ>::PITCH;
-    auto kern = plane_kernel<NY, NZ, NTHR, MINB, INV, Load, Store>;
+    auto kern = plane_kernel<NY, NZ, NTHR, MINB, INV, DB1, DB2, Load, Store>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    dim3 grid((unsigned)(a.npencils / NY), (unsigned)a.batch);
-    kern<<<grid, NTHR, smem, s>>>(ld, st, a.tw2, a.tw);
+    const int nx = (int)(a.npencils / NY), nunits = nx * a.batch;
+    static int resident = 0;                                  // CTAs the device holds at once
+    if (!resident) {
+        int dev = 0, sms = 0, per_sm = 0;
+        cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NTHR, smem);
+        resident = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    const int var = plane_variant();
+    const int grid = (var & 1) ? (nunits < resident ? nunits : resident) : nunits;
+    kern<<<grid, NTHR, smem, s>>>(ld, st, nx, nunits, (var & 8) ? 1 : 0, a.tw2, a.tw);
     return cudaGetLastError();
+}
+template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
+static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
+    const int var = plane_variant();
+    if (NY == 72) {
+        switch ((var >> 1) & 3) {
+            case 1: return plane_launch2<NY, NZ, NTHR, MINB, INV, true, false>(ld, st, a, s);
+            case 2: return plane_launch2<NY, NZ, NTHR, MINB, INV, false, true>(ld, st, a, s);
+            case 3: return plane_launch2<NY, NZ, NTHR, MINB, INV, true, true>(ld, st, a, s);
+            default: break;
+        }
+    }
+    return plane_launch2<NY, NZ, NTHR, MINB, INV, false, false>(ld, st, a, s);
 }
 template <int NY, int NZ, int NTHR, int MINB>
 static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {

@@ -35,26 +35,46 @@ template <int R1> __device__ __forceinline__ void load_twiddles(const cplx* __re
     for (int r = 1; r < R1; ++r) w[r] = __ldg(&tw[i * r]);
 }
 
-// ---- bound load / store functors: per-CTA state resolved once ----------------------------------------------
-struct BLoadWork { const cplx* g; __device__ __forceinline__ cplx operator()(long idx) const { return g[idx]; } };
+// ---- bound load / store functors: per-unit state resolved once; loads are split into fetch (issue the global
+// loads, keep the raw operands in registers) and make (combine them), so that a round's loads can be issued one
+// round ahead of their use ---------------------------------------------------------------------------------------
+struct BLoadWork {
+    const cplx* g;
+    typedef cplx Raw;
+    __device__ __forceinline__ Raw fetch(long idx) const { return g[idx]; }
+    __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
+    __device__ __forceinline__ void prefetch_l2(long, int, int, int) const {}
+};
 struct BStoreWork { cplx* g; __device__ __forceinline__ void operator()(long idx, cplx v) const { g[idx] = v; } };
 struct BLoadPair {
     const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = b0*b1 (b0 null: im = 0)
-    __device__ __forceinline__ cplx operator()(long idx) const {
-        const double re = __ldg(a0 + idx) * __ldg(a1 + idx);
-        const double im = b0 ? __ldg(b0 + idx) * __ldg(b1 + idx) : 0.0;
-        return make_double2(re, im);
+    struct Raw { double p, q, r, s; };
+    __device__ __forceinline__ Raw fetch(long idx) const {
+        Raw w; w.p = __ldg(a0 + idx); w.q = __ldg(a1 + idx);
+        if (b0) { w.r = __ldg(b0 + idx); w.s = __ldg(b1 + idx); } else { w.r = 0.0; w.s = 0.0; }
+        return w;
+    }
+    __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2(w.p * w.q, w.r * w.s); }
+    // pull the operand planes [base, base + n) of the unit this CTA handles next into L2 (no registers held)
+    __device__ __forceinline__ void prefetch_l2(long base, int n, int tid, int nthr) const {
+        for (int e = tid * 16; e < n; e += nthr * 16) {          // one 128-byte line = 16 doubles
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a0 + base + e));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a1 + base + e));
+            if (b0) { asm volatile("prefetch.global.L2 [%0];" ::"l"(b0 + base + e)); asm volatile("prefetch.global.L2 [%0];" ::"l"(b1 + base + e)); }
+        }
     }
 };
 struct BLoadPack2 {
     const double* s0; const double* s1; BatchLayout lay; long f; bool has_im; double scale;
-    __device__ __forceinline__ cplx operator()(long idx) const {
+    struct Raw { double p, q, r, s; };
+    __device__ __forceinline__ Raw fetch(long idx) const {
         const long o0 = lay(f, idx);
-        double re = s0[o0]; if (s1) re += s1[o0];
-        double im = 0.0;
-        if (has_im) { const long o1 = o0 + lay.next(); im = s0[o1]; if (s1) im += s1[o1]; }
-        return make_double2(re * scale, im * scale);
+        Raw w; w.p = s0[o0]; w.q = s1 ? s1[o0] : 0.0; w.r = 0.0; w.s = 0.0;
+        if (has_im) { const long o1 = o0 + lay.next(); w.r = s0[o1]; if (s1) w.s = s1[o1]; }
+        return w;
     }
+    __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2((w.p + w.q) * scale, (w.r + w.s) * scale); }
+    __device__ __forceinline__ void prefetch_l2(long, int, int, int) const {}
 };
 struct BStoreSplit2 {
     double* dst; BatchLayout lay; long f; bool has_im; double scale;
@@ -75,127 +95,201 @@ __device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b) {
 __device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b) { return BLoadPack2{l.src0, l.src1, l.lay, 2L * b, 2 * b + 1 < l.nfun, l.scale}; }
 __device__ __forceinline__ BStoreSplit2 bind(const StoreSplit2& s, int b) { return BStoreSplit2{s.dst, s.lay, 2L * b, 2 * b + 1 < s.nfun, s.scale}; }
 
+// One phase = ITEMS butterflies spread over the CTA in rounds of NTHR.  The loads of round r+1 are issued before
+// round r is computed and stored (double-buffered registers), so memory latency overlaps the butterflies.
+// load(t, buf) fills buf for item t; work(t, buf) computes and stores item t.
+template <int ITEMS, int NTHR, bool DB, class Buf, class LoadF, class WorkF>
+__device__ __forceinline__ void run_rounds(int tid, LoadF&& load, WorkF&& work) {
+    constexpr int NR = (ITEMS + NTHR - 1) / NTHR;
+    if constexpr (DB) {
+        Buf cur, nxt;
+        if (tid < ITEMS) load(tid, cur);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            const int t = tid + r * NTHR;
+            if (r + 1 < NR && t + NTHR < ITEMS) load(t + NTHR, nxt);
+            if (t < ITEMS) work(t, cur);
+            if (r + 1 < NR) cur = nxt;
+        }
+    } else {
+        for (int t = tid; t < ITEMS; t += NTHR) { Buf cur; load(t, cur); work(t, cur); }
+    }
+}
+template <class T, int R> struct RegBuf { T v[R]; };
+// registers per thread that still let MINB CTAs of NTHR threads share the 64 K register file (warp granularity 8 regs)
+template <int NTHR, int MINB> struct PlaneRegs {
+    static constexpr int warps = (NTHR + 31) / 32 * MINB;
+    static constexpr int raw = 65536 / (warps * 32) / 8 * 8;
+    static constexpr int value = raw > 255 ? 255 : raw;
+};
+
 // ---- plane kernel -------------------------------------------------------------------------------------------
-// grid = (NX planes, batch).  Flat index of (x, y, z) inside a grid: (x*NY + y)*NZ + z.
-template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
-__global__ void __launch_bounds__(NTHR, MINB) plane_kernel(Load ld, Store st, const cplx* __restrict__ twy_g, const cplx* __restrict__ twz_g) {
+// Persistent CTAs walk over the units (packed grid b, plane x), unit u = b*NX + x.  Flat index of (x, y, z) inside
+// a grid: (x*NY + y)*NZ + z.
+template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
+__global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::value)) plane_kernel(Load ld, Store st, int nx, int nunits, int l2pf, const cplx* __restrict__ twy_g, const cplx* __restrict__ twz_g) {
     using TY = Two<NY>; using TZ = Two<NZ>;
     constexpr int R1y = TY::R1, R2y = TY::R2, R1z = TZ::R1, R2z = TZ::R2;
     constexpr int PITCH = TZ::PITCH;
-    constexpr bool ZFIX = (NTHR % R2z == 0), YFIX = (NTHR % R2y == 0);     // residue i = tid % R2 is the same in every round
+    static_assert(NTHR % R2z == 0 && NTHR % R2y == 0, "a thread's residue must be the same in every round");
     extern __shared__ cplx sm[];
     const int tid = threadIdx.x;
-    const long pbase = (long)blockIdx.x * NY * NZ;
-    const auto L = bind(ld, (int)blockIdx.y);
-    const auto S = bind(st, (int)blockIdx.y);
     cplx wz[R1z], wy[R1y];
-    if (ZFIX) load_twiddles<R1z>(twz_g, tid % R2z, wz);
-    if (YFIX) load_twiddles<R1y>(twy_g, tid % R2y, wy);
+    load_twiddles<R1z>(twz_g, tid % R2z, wz);
+    if constexpr (NY == NZ) {
+#pragma unroll
+        for (int r = 0; r < R1y; ++r) wy[r] = wz[r];
+    } else load_twiddles<R1y>(twy_g, tid % R2y, wy);
+    typedef decltype(bind(ld, 0)) BL;
+    typedef typename BL::Raw Raw;
 
-    if constexpr (!INV) {
-        // z stage 1 (radix R1z, twiddle after): global -> registers -> shared
-        for (int t = tid; t < NY * R2z; t += NTHR) {
-            const int y = t / R2z, i = t - y * R2z;
-            if (!ZFIX) load_twiddles<R1z>(twz_g, i, wz);
-            cplx x[R1z];
-#pragma unroll
-            for (int r = 0; r < R1z; ++r) x[r] = L(pbase + y * NZ + i + R2z * r);
-            Dft<R1z, false>::run(x);
-            cplx* row = sm + y * PITCH;
-            row[TZ::pad(i)] = x[0];
-#pragma unroll
-            for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], wz[k]);
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
+        const int b = u / nx;
+        const long pbase = (long)(u - b * nx) * NY * NZ;
+        const BL L = bind(ld, b);
+        const auto S = bind(st, b);
+        {   // operands of the unit this CTA takes next -> L2
+            const int un = u + gridDim.x;
+            if (l2pf && un < nunits) { const int bn = un / nx; bind(ld, bn).prefetch_l2((long)(un - bn * nx) * NY * NZ, NY * NZ, tid, NTHR); }
         }
-        __syncthreads();
-        // z stage 2 (radix R2z on blocks of R2z consecutive positions), in place
-        for (int t = tid; t < NY * R1z; t += NTHR) {
-            const int y = t / R1z, k1 = t - y * R1z;
-            cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
-            cplx x[R2z];
+        if constexpr (!INV) {
+            // z stage 1 (radix R1z, twiddle after): global -> registers -> shared
+            run_rounds<NY * R2z, NTHR, DB1, RegBuf<Raw, R1z>>(tid,
+                [&](int t, RegBuf<Raw, R1z>& q) {
+                    const int y = t / R2z, i = t - y * R2z;
 #pragma unroll
-            for (int i = 0; i < R2z; ++i) x[i] = blk[i];
-            Dft<R2z, false>::run(x);
+                    for (int r = 0; r < R1z; ++r) q.v[r] = L.fetch(pbase + y * NZ + i + R2z * r);
+                },
+                [&](int t, const RegBuf<Raw, R1z>& q) {
+                    const int y = t / R2z, i = t - y * R2z;
+                    cplx x[R1z];
 #pragma unroll
-            for (int i = 0; i < R2z; ++i) blk[i] = x[i];
+                    for (int r = 0; r < R1z; ++r) x[r] = L.make(q.v[r]);
+                    Dft<R1z, false>::run(x);
+                    cplx* row = sm + y * PITCH;
+                    row[TZ::pad(i)] = x[0];
+#pragma unroll
+                    for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], wz[k]);
+                });
+            __syncthreads();
+            // z stage 2 (radix R2z on blocks of R2z consecutive positions), in place
+            run_rounds<NY * R1z, NTHR, DB2, RegBuf<cplx, R2z>>(tid,
+                [&](int t, RegBuf<cplx, R2z>& q) {
+                    const int y = t / R1z, k1 = t - y * R1z;
+                    const cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
+#pragma unroll
+                    for (int i = 0; i < R2z; ++i) q.v[i] = blk[i];
+                },
+                [&](int t, RegBuf<cplx, R2z>& q) {
+                    const int y = t / R1z, k1 = t - y * R1z;
+                    cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
+                    Dft<R2z, false>::run(q.v);
+#pragma unroll
+                    for (int i = 0; i < R2z; ++i) blk[i] = q.v[i];
+                });
+            __syncthreads();
+            // y stage 1 (radix R1y, twiddle after): lanes run over the residue i, the odd pitch keeps them on distinct banks
+            run_rounds<NZ * R2y, NTHR, DB2, RegBuf<cplx, R1y>>(tid,
+                [&](int t, RegBuf<cplx, R1y>& q) {
+                    const int zp = t / R2y, i = t - zp * R2y;
+                    const cplx* col = sm + TZ::pad(zp) + i * PITCH;
+#pragma unroll
+                    for (int r = 0; r < R1y; ++r) q.v[r] = col[r * R2y * PITCH];
+                },
+                [&](int t, RegBuf<cplx, R1y>& q) {
+                    const int zp = t / R2y, i = t - zp * R2y;
+                    cplx* col = sm + TZ::pad(zp) + i * PITCH;
+                    Dft<R1y, false>::run(q.v);
+                    col[0] = q.v[0];
+#pragma unroll
+                    for (int k = 1; k < R1y; ++k) col[k * R2y * PITCH] = cmul(q.v[k], wy[k]);
+                });
+            __syncthreads();
+            // y stage 2 (radix R2y): shared -> registers -> global, lanes run over z (coalesced rows)
+            run_rounds<NZ * R1y, NTHR, DB2, RegBuf<cplx, R2y>>(tid,
+                [&](int t, RegBuf<cplx, R2y>& q) {
+                    const int k1 = t / NZ, zp = t - k1 * NZ;
+                    const cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
+#pragma unroll
+                    for (int i = 0; i < R2y; ++i) q.v[i] = col[i * PITCH];
+                },
+                [&](int t, RegBuf<cplx, R2y>& q) {
+                    const int k1 = t / NZ, zp = t - k1 * NZ;
+                    Dft<R2y, false>::run(q.v);
+#pragma unroll
+                    for (int k = 0; k < R2y; ++k) S(pbase + (long)(k1 * R2y + k) * NZ + zp, q.v[k]);
+                });
+        } else {
+            // y inverse stage R2y: global -> registers -> shared
+            run_rounds<NZ * R1y, NTHR, DB1, RegBuf<Raw, R2y>>(tid,
+                [&](int t, RegBuf<Raw, R2y>& q) {
+                    const int k1 = t / NZ, zp = t - k1 * NZ;
+#pragma unroll
+                    for (int i = 0; i < R2y; ++i) q.v[i] = L.fetch(pbase + (long)(k1 * R2y + i) * NZ + zp);
+                },
+                [&](int t, const RegBuf<Raw, R2y>& q) {
+                    const int k1 = t / NZ, zp = t - k1 * NZ;
+                    cplx x[R2y];
+#pragma unroll
+                    for (int i = 0; i < R2y; ++i) x[i] = L.make(q.v[i]);
+                    Dft<R2y, true>::run(x);
+                    cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
+#pragma unroll
+                    for (int i = 0; i < R2y; ++i) col[i * PITCH] = x[i];
+                });
+            __syncthreads();
+            // y inverse stage R1y (conjugate twiddle before the butterfly), in place
+            run_rounds<NZ * R2y, NTHR, DB2, RegBuf<cplx, R1y>>(tid,
+                [&](int t, RegBuf<cplx, R1y>& q) {
+                    const int zp = t / R2y, i = t - zp * R2y;
+                    const cplx* col = sm + TZ::pad(zp) + i * PITCH;
+#pragma unroll
+                    for (int k = 0; k < R1y; ++k) q.v[k] = col[k * R2y * PITCH];
+                },
+                [&](int t, RegBuf<cplx, R1y>& q) {
+                    const int zp = t / R2y, i = t - zp * R2y;
+                    cplx* col = sm + TZ::pad(zp) + i * PITCH;
+#pragma unroll
+                    for (int k = 1; k < R1y; ++k) q.v[k] = cmulc(q.v[k], wy[k]);
+                    Dft<R1y, true>::run(q.v);
+#pragma unroll
+                    for (int r = 0; r < R1y; ++r) col[r * R2y * PITCH] = q.v[r];
+                });
+            __syncthreads();
+            // z inverse stage R2z, in place
+            run_rounds<NY * R1z, NTHR, DB2, RegBuf<cplx, R2z>>(tid,
+                [&](int t, RegBuf<cplx, R2z>& q) {
+                    const int y = t / R1z, k1 = t - y * R1z;
+                    const cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
+#pragma unroll
+                    for (int i = 0; i < R2z; ++i) q.v[i] = blk[i];
+                },
+                [&](int t, RegBuf<cplx, R2z>& q) {
+                    const int y = t / R1z, k1 = t - y * R1z;
+                    cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
+                    Dft<R2z, true>::run(q.v);
+#pragma unroll
+                    for (int i = 0; i < R2z; ++i) blk[i] = q.v[i];
+                });
+            __syncthreads();
+            // z inverse stage R1z: shared -> registers -> global (natural order)
+            run_rounds<NY * R2z, NTHR, DB2, RegBuf<cplx, R1z>>(tid,
+                [&](int t, RegBuf<cplx, R1z>& q) {
+                    const int y = t / R2z, i = t - y * R2z;
+                    const cplx* row = sm + y * PITCH;
+#pragma unroll
+                    for (int k = 0; k < R1z; ++k) q.v[k] = row[TZ::pad(i + R2z * k)];
+                },
+                [&](int t, RegBuf<cplx, R1z>& q) {
+                    const int y = t / R2z, i = t - y * R2z;
+#pragma unroll
+                    for (int k = 1; k < R1z; ++k) q.v[k] = cmulc(q.v[k], wz[k]);
+                    Dft<R1z, true>::run(q.v);
+#pragma unroll
+                    for (int r = 0; r < R1z; ++r) S(pbase + y * NZ + i + R2z * r, q.v[r]);
+                });
         }
-        __syncthreads();
-        // y stage 1 (radix R1y, twiddle after): lanes run over the residue i, the odd pitch keeps them on distinct banks
-        for (int t = tid; t < NZ * R2y; t += NTHR) {
-            const int zp = t / R2y, i = t - zp * R2y;
-            if (!YFIX) load_twiddles<R1y>(twy_g, i, wy);
-            cplx* col = sm + TZ::pad(zp) + i * PITCH;
-            cplx x[R1y];
-#pragma unroll
-            for (int r = 0; r < R1y; ++r) x[r] = col[r * R2y * PITCH];
-            Dft<R1y, false>::run(x);
-            col[0] = x[0];
-#pragma unroll
-            for (int k = 1; k < R1y; ++k) col[k * R2y * PITCH] = cmul(x[k], wy[k]);
-        }
-        __syncthreads();
-        // y stage 2 (radix R2y): shared -> registers -> global, lanes run over z (coalesced rows)
-        for (int t = tid; t < NZ * R1y; t += NTHR) {
-            const int k1 = t / NZ, zp = t - k1 * NZ;
-            const cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
-            cplx x[R2y];
-#pragma unroll
-            for (int i = 0; i < R2y; ++i) x[i] = col[i * PITCH];
-            Dft<R2y, false>::run(x);
-#pragma unroll
-            for (int k = 0; k < R2y; ++k) S(pbase + (long)(k1 * R2y + k) * NZ + zp, x[k]);
-        }
-    } else {
-        // y inverse stage R2y: global -> registers -> shared
-        for (int t = tid; t < NZ * R1y; t += NTHR) {
-            const int k1 = t / NZ, zp = t - k1 * NZ;
-            cplx x[R2y];
-#pragma unroll
-            for (int i = 0; i < R2y; ++i) x[i] = L(pbase + (long)(k1 * R2y + i) * NZ + zp);
-            Dft<R2y, true>::run(x);
-            cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
-#pragma unroll
-            for (int i = 0; i < R2y; ++i) col[i * PITCH] = x[i];
-        }
-        __syncthreads();
-        // y inverse stage R1y (conjugate twiddle before the butterfly), in place
-        for (int t = tid; t < NZ * R2y; t += NTHR) {
-            const int zp = t / R2y, i = t - zp * R2y;
-            if (!YFIX) load_twiddles<R1y>(twy_g, i, wy);
-            cplx* col = sm + TZ::pad(zp) + i * PITCH;
-            cplx x[R1y];
-            x[0] = col[0];
-#pragma unroll
-            for (int k = 1; k < R1y; ++k) x[k] = cmulc(col[k * R2y * PITCH], wy[k]);
-            Dft<R1y, true>::run(x);
-#pragma unroll
-            for (int r = 0; r < R1y; ++r) col[r * R2y * PITCH] = x[r];
-        }
-        __syncthreads();
-        // z inverse stage R2z, in place
-        for (int t = tid; t < NY * R1z; t += NTHR) {
-            const int y = t / R1z, k1 = t - y * R1z;
-            cplx* blk = sm + y * PITCH + TZ::pad(k1 * R2z);
-            cplx x[R2z];
-#pragma unroll
-            for (int i = 0; i < R2z; ++i) x[i] = blk[i];
-            Dft<R2z, true>::run(x);
-#pragma unroll
-            for (int i = 0; i < R2z; ++i) blk[i] = x[i];
-        }
-        __syncthreads();
-        // z inverse stage R1z: shared -> registers -> global (natural order)
-        for (int t = tid; t < NY * R2z; t += NTHR) {
-            const int y = t / R2z, i = t - y * R2z;
-            if (!ZFIX) load_twiddles<R1z>(twz_g, i, wz);
-            const cplx* row = sm + y * PITCH;
-            cplx x[R1z];
-            x[0] = row[TZ::pad(i)];
-#pragma unroll
-            for (int k = 1; k < R1z; ++k) x[k] = cmulc(row[TZ::pad(i + R2z * k)], wz[k]);
-            Dft<R1z, true>::run(x);
-#pragma unroll
-            for (int r = 0; r < R1z; ++r) S(pbase + y * NZ + i + R2z * r, x[r]);
-        }
+        __syncthreads();        // the plane buffer is reused by the next unit
     }
 }
 

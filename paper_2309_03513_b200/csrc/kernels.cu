@@ -1,4 +1,5 @@
 // Pointwise, scatter/gather, contraction and LDA kernels of the Liouville hot path (hand-written CUDA, sm_100a).
+#include <cstdlib>
 #include "kernels.h"
 
 namespace tddft {
@@ -150,10 +151,8 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-constexpr int CT_PITCH = CHUNK + 2;                // padded row pitch (doubles): 272 bytes
 constexpr int CT_AROWS = 128;                      // tau rows per stage: 32 rows x 4 columns
 constexpr int CT_STAGES = 4;
-constexpr int CT_WARPS = 16;                       // 2 grid points each
 struct ColSweep {        // the column starts (multiples of 4) a unit visits: blocks of 32 in skewed order, empty blocks skipped
     int t, cs, cend, wb, dir, ncols;
     __device__ void settle() {
@@ -172,18 +171,26 @@ struct ColSweep {        // the column starts (multiples of 4) a unit visits: bl
 // DUAL = true: off-diagonal tile, dense slots slot(i,j) = i*tj + j, units 0-3 = direction 1, 4-7 = direction 2.
 // DUAL = false: diagonal tile (ti == tj, same orbital block): one direction, tau stored for i <= j only, packed
 // row-major (the order build_tiles emits the pairs), read symmetrically.
-template <int NK, bool DUAL>
-__global__ void __launch_bounds__(32 * CT_WARPS, 1)
+// WARPS warps of 2 grid points each: one CTA owns 2*WARPS points of a chunk (WARPS = 8: half a chunk, two CTAs per SM,
+// so one CTA's pipeline fill and write-back overlap the other's DMMA loop).  The accumulators start from -out/alpha
+// (loaded while the ring fills), so the write-back is store-only.
+template <int NK, bool DUAL, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 16 / WARPS)
 contract_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau, const int* __restrict__ slot,
                 const double* __restrict__ zeros, int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
     extern __shared__ __align__(16) double sm[];
+    constexpr int PTS = 2 * WARPS;                         // grid points per CTA
+    constexpr int PARTS = CHUNK / PTS;                     // CTAs that share a chunk
+    constexpr int PITCH = PTS + 2;                         // padded row pitch (doubles): conflict-free 16-byte fragment reads
     constexpr int BROWS = 4 * 8 * NK;                      // rows of a per stage: 4 columns x (8*NK) trial vectors
     constexpr int ROWS = CT_AROWS + BROWS;
-    constexpr int STAGE = ROWS * CT_PITCH;                 // doubles
-    constexpr int NCOPY = ROWS / 32;                       // 16-byte copies per thread per stage (512 threads x 16 B = 32 rows)
+    constexpr int STAGE = ROWS * PITCH;                    // doubles
+    constexpr int NCOPY = ROWS / 32;                       // 16-byte copies per thread per stage (32 rows per pass)
     constexpr int NCOPY_A = CT_AROWS / 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const long chunk = blockIdx.x >> 3;
+    const long cidx = blockIdx.x >> 3;
+    const long chunk = cidx / PARTS;
+    const int pt0 = (int)(cidx % PARTS) * PTS;             // first point of this CTA inside the chunk
     const int unit = blockIdx.x & 7;
     const int dir = DUAL ? (unit >> 2) : 0;
     const int wb = DUAL ? (unit & 3) : (int)(blockIdx.y * 8 + unit);
@@ -191,14 +198,13 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
     const int rowf0 = dir == 0 ? i0 : j0, colf0 = dir == 0 ? j0 : i0;
     const int rb = wb * 32;
     if (rb >= nrows) return;
-    const double* tau_c = tau + chunk * stot * CHUNK;
-    const double* a_c = a + chunk * ftot * CHUNK;
-    // this thread's copies: copy q moves piece (tid & 15) of stage row rc = q*32 + (tid >> 4)
-    const int piece2 = (tid & 15) * 2;
-    const int rsub = tid >> 4;                             // 0..31
+    const double* tau_c = tau + chunk * stot * CHUNK + pt0;
+    const double* a_c = a + chunk * ftot * CHUNK + pt0;
+    // this thread's copies: copy q moves piece (tid % WARPS) of stage row rc = q*32 + tid / WARPS
+    const int piece2 = (tid % WARPS) * 2;
+    const int rsub = tid / WARPS;                          // 0..31
     const long a_colstride = (long)kc * CHUNK;             // next column of a
-    // out-of-range rows and columns are zero-filled with plain shared-memory stores (never read from a shared global
-    // zero line: thousands of CTAs hammering one line serialise in L2)
+    // out-of-range rows and columns are zero-filled with plain shared-memory stores
     auto load_stage = [&](int buf, int cs) {
         double* base = sm + buf * STAGE;
 #pragma unroll
@@ -221,7 +227,7 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
                 const int k = qq >> 2, col = cs + (qq & 3);
                 if (col < ncols && k < kn) src = a_c + (long)(colf0 + col) * a_colstride + (long)k * CHUNK + piece2;
             }
-            double* dst = base + rc * CT_PITCH + piece2;
+            double* dst = base + rc * PITCH + piece2;
             if (src) cp_async16(dst, src);
             else *(double2*)dst = make_double2(0.0, 0.0);
         }
@@ -230,17 +236,27 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
     issue.init(dir, DUAL ? wb : 0, ncols);
     use = issue;
     const int lr = lane >> 2, lc = lane & 3;
-    double acc[4][NK][2][2];
-#pragma unroll
-    for (int m = 0; m < 4; ++m)
-#pragma unroll
-        for (int n = 0; n < NK; ++n)
-#pragma unroll
-            for (int q = 0; q < 2; ++q) acc[m][n][q][0] = acc[m][n][q][1] = 0.0;
 #pragma unroll
     for (int st = 0; st < CT_STAGES - 1; ++st) {
         if (issue.valid()) { load_stage(st, issue.cs); issue.next(); }
         cp_async_commit();
+    }
+    // accumulators start from -out/alpha while the ring fills
+    double acc[4][NK][2][2];
+    double* out_c = out + chunk * ftot * CHUNK + pt0 + warp * 2;
+    const double minv = -1.0 / alpha;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        const int i = rb + m * 8 + lr;
+#pragma unroll
+        for (int n = 0; n < NK; ++n)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int k = n * 8 + 2 * lc + h;
+                double2 x = make_double2(0.0, 0.0);
+                if (i < nrows && k < kn) x = *(const double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK);
+                acc[m][n][0][h] = x.x * minv; acc[m][n][1][h] = x.y * minv;
+            }
     }
     for (int step = 0; use.valid(); use.next(), ++step) {
         const int buf = step % CT_STAGES;
@@ -249,12 +265,12 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
         if (issue.valid()) { load_stage((step + CT_STAGES - 1) % CT_STAGES, issue.cs); issue.next(); }
         cp_async_commit();
         const double* As = sm + buf * STAGE + warp * 2;
-        const double* Bs = As + CT_AROWS * CT_PITCH;
+        const double* Bs = As + CT_AROWS * PITCH;
         double2 af[4], bf[NK];
 #pragma unroll
-        for (int m = 0; m < 4; ++m) af[m] = *(const double2*)(As + ((m * 8 + lr) * 4 + lc) * CT_PITCH);
+        for (int m = 0; m < 4; ++m) af[m] = *(const double2*)(As + ((m * 8 + lr) * 4 + lc) * PITCH);
 #pragma unroll
-        for (int n = 0; n < NK; ++n) bf[n] = *(const double2*)(Bs + ((n * 8 + lr) * 4 + lc) * CT_PITCH);
+        for (int n = 0; n < NK; ++n) bf[n] = *(const double2*)(Bs + ((n * 8 + lr) * 4 + lc) * PITCH);
 #pragma unroll
         for (int m = 0; m < 4; ++m)
 #pragma unroll
@@ -264,7 +280,7 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
             }
     }
     cp_async_wait<0>();
-    double* out_c = out + chunk * ftot * CHUNK + warp * 2;
+    const double malpha = -alpha;
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         const int i = rb + m * 8 + lr;
@@ -275,26 +291,35 @@ contract_kernel(double* __restrict__ out, const double* __restrict__ a, const do
             for (int h = 0; h < 2; ++h) {
                 const int k = n * 8 + 2 * lc + h;
                 if (k >= kn) continue;
-                double2* op = (double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK);
-                double2 x = *op;
-                x.x = fma(-alpha, acc[m][n][0][h], x.x); x.y = fma(-alpha, acc[m][n][1][h], x.y);
-                *op = x;
+                *(double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK) = make_double2(malpha * acc[m][n][0][h], malpha * acc[m][n][1][h]);
             }
     }
 }
 
-template <int NK, bool DUAL>
-static cudaError_t contract_launch(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
-                                   int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    const size_t smem = sizeof(double) * CT_STAGES * (CT_AROWS + 4 * 8 * NK) * CT_PITCH;
+static int contract_warps() {      // points per CTA = 2 * warps: 8 (two CTAs per SM, default) or 16
+    static int w = 0;
+    if (!w) { const char* e = getenv("TDDFT_CT_WARPS"); w = (e && atoi(e) == 16) ? 16 : 8; }
+    return w;
+}
+template <int NK, bool DUAL, int WARPS>
+static cudaError_t contract_launch2(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
+                                    int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
+    const size_t smem = sizeof(double) * CT_STAGES * (CT_AROWS + 4 * 8 * NK) * (2 * WARPS + 2);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(contract_kernel<NK, DUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(contract_kernel<NK, DUAL, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    contract_kernel<NK, DUAL><<<grid, 32 * CT_WARPS, smem, st>>>(out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
+    grid.x *= CHUNK / (2 * WARPS);
+    contract_kernel<NK, DUAL, WARPS><<<grid, 32 * WARPS, smem, st>>>(out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
     return cudaGetLastError();
+}
+template <int NK, bool DUAL>
+static cudaError_t contract_launch(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
+                                   int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
+    if (contract_warps() == 16) return contract_launch2<NK, DUAL, 16>(grid, out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
+    return contract_launch2<NK, DUAL, 8>(grid, out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
 }
 cudaError_t launch_contract_single(double* out, const double* a, const double* tau, const int* slot, const double* zeros, int i0, int ti,
                                    int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st) {

@@ -274,13 +274,13 @@ def main():
     peak, peak_src = measured_peaks()
     s4_ms = stage_ms.get("ms_s4_pair_fft", 0.0)
     pairs_per_step = pair_ffts / max(args.steps, 1)
-    fft_batch = args.fft_batch or max(1, min(64, (192 << 20) // (16 * nr)))
+    fft_batch = st["fft_batch"]
     roofline = None
     if s4_ms > 0 and pair_ffts > 0:
         bytes_per_pair = 32.0 * nr                      # one HBM round trip per direction per pair density
         achieved = pair_ffts * bytes_per_pair / (s4_ms * 1e-3) / 1e9
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                    "traffic": None, "kernel": "S4 pair-FFT pipeline (zpass/spass kernels, 5 launches per batch of %d pairs)" % (2 * fft_batch),
+                    "traffic": None, "kernel": "S4 pair-FFT pipeline (%s, batches of %d pairs)" % ("plane_kernel fwd + xpass_kernel conv + plane_kernel inv" if st["fft_path"] == 0 else "5 general pass kernels", 2 * fft_batch),
                     "algorithmic_bytes_per_pair": bytes_per_pair, "peak_source": peak_src,
                     "share_of_step": s4_ms / max(stage_ms.get("ms_total", 1e-9), 1e-9)}
     cpu_baseline = None

@@ -425,7 +425,19 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         } else c->fused = true;
         c->fused = c->fused && fused_supported(grid);
         const long nr = c->hp.nr, npwh = c->hp.npwh;
-        if (c->fft_batch <= 0) c->fft_batch = (int)std::max<long>(1, std::min<long>(64, (192L << 20) / (16 * nr)));   // latency-bound kernels: large launches beat L2 residency (measured)
+        if (c->fft_batch <= 0) {
+            // latency-bound kernels: large launches beat L2 residency (measured); among the sizes up to 64 grids and 256 MB
+            // take the one whose plane units (n1 per grid) fill whole waves of two CTAs per SM
+            const long cap = std::max<long>(1, std::min<long>(64, (256L << 20) / (16 * nr)));
+            const long resident = 2L * c->num_sms;
+            long bestb = cap; double beste = 0.0;
+            for (long b = cap; b >= std::max<long>(1, cap / 2); --b) {
+                const long units = b * grid[0], waves = (units + resident - 1) / resident;
+                const double e = (double)units / (double)(waves * resident);
+                if (e > beste + 0.01) { beste = e; bestb = b; }
+            }
+            c->fft_batch = (int)bestb;
+        }
 #define INIT_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? TDDFT_ENOMEM : TDDFT_ECUDA, std::string("init: " #call ": ") + cudaGetErrorString(e_)); } while (0)
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_p, sizeof(int) * npwh));
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_m, sizeof(int) * npwh));
@@ -514,7 +526,11 @@ int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int 
 }
 
 int tddft_set_timing(tddft_ctx* c, int enabled) { if (!c) return TDDFT_EINVAL; c->timing = enabled != 0; return TDDFT_OK; }
-int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) { if (!c || !out) return TDDFT_EINVAL; *out = c->stats; return TDDFT_OK; }
+int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) {
+    if (!c || !out) return TDDFT_EINVAL;
+    *out = c->stats; out->fft_batch = c->fft_batch; out->fft_path = c->fused ? 0 : 1;
+    return TDDFT_OK;
+}
 
 int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs, double* tau) {
     if (!c || !pairs || !tau || n_pairs < 0 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;

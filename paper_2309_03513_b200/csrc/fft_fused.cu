@@ -9,7 +9,7 @@ namespace tddft {
 #define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8)
 #define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
 
-static int plane_variant() {          // experiment switch: bit0 persistent grid, bit1 DB1, bit2 DB2, bit3 L2 prefetch
+static int plane_variant() {          // tuning switch TDDFT_VAR: bit 0 persistent grid, bit 3 L2 prefetch of the next unit's operands (default both)
     static int v = -1;
     if (v < 0) { const char* e = getenv("TDDFT_VAR"); v = e ? atoi(e) : 9; }
     return v;
@@ -40,15 +40,7 @@ static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t
 }
 template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
 static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
-    const int var = plane_variant();
-    if (NY == 72) {
-        switch ((var >> 1) & 3) {
-            case 1: return plane_launch2<NY, NZ, NTHR, MINB, INV, true, false>(ld, st, a, s);
-            case 2: return plane_launch2<NY, NZ, NTHR, MINB, INV, false, true>(ld, st, a, s);
-            case 3: return plane_launch2<NY, NZ, NTHR, MINB, INV, true, true>(ld, st, a, s);
-            default: break;
-        }
-    }
+    // double-buffered rounds (DB1 / DB2 of plane_kernel) measured slower on B200 (register pressure): both off
     return plane_launch2<NY, NZ, NTHR, MINB, INV, false, false>(ld, st, a, s);
 }
 template <int NY, int NZ, int NTHR, int MINB>
@@ -77,7 +69,26 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    dim3 grid((unsigned)((a.inner + XW - 1) / XW), (unsigned)a.batch);
+    // batch groups: enough CTAs for ~6 waves of the resident set, each CTA keeps its twiddles and Coulomb-table values
+    // in registers while it walks over its grids
+    const unsigned tiles = (unsigned)((a.inner + XW - 1) / XW);
+    static int resident = 0;
+    if (!resident) {
+        int dev = 0, sms = 0, per_sm = 0;
+        cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_kernel<NX, SM_CONV>, XCfg<NX>::NTHR, smem);
+        resident = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    int gy = a.batch, best_gy = a.batch; double best = 0.0;
+    for (gy = 1; gy <= a.batch; ++gy) {
+        if ((long)tiles * gy < 3L * resident && gy < a.batch) continue;      // at least 3 waves (or one grid per CTA)
+        const long ctas = (long)tiles * gy, waves = (ctas + resident - 1) / resident;
+        const int per = (a.batch + gy - 1) / gy;                              // grids per CTA: imbalance when batch % gy != 0
+        const double eff = (double)ctas / (double)(waves * resident) * (double)a.batch / (double)(per * gy);
+        if (eff > best + 1e-9) { best = eff; best_gy = gy; }
+    }
+    { static int force = -1; if (force < 0) { const char* e = getenv("TDDFT_XGY"); force = e ? atoi(e) : 0; } if (force > 0) best_gy = force < a.batch ? force : a.batch; }
+    dim3 grid(tiles, (unsigned)best_gy);
     constexpr int NT = XCfg<NX>::NTHR;
     if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab);
     else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab);

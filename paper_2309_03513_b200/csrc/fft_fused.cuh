@@ -41,33 +41,42 @@ template <int R1> __device__ __forceinline__ void load_twiddles(const cplx* __re
 struct BLoadWork {
     const cplx* g;
     typedef cplx Raw;
-    __device__ __forceinline__ Raw fetch(long idx) const { return g[idx]; }
+    static constexpr int kModes = 1;
+    __device__ __forceinline__ int mode() const { return 0; }
+    template <int M> __device__ __forceinline__ Raw fetch(long idx) const { return g[idx]; }
     __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
     __device__ __forceinline__ void prefetch_l2(long, int, int, int) const {}
 };
 struct BStoreWork { cplx* g; __device__ __forceinline__ void operator()(long idx, cplx v) const { g[idx] = v; } };
 struct BLoadPair {
-    const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = b0*b1 (b0 null: im = 0)
+    const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = imw*b0*b1 (imw = 0 for the odd last pair, which reuses a0, a1)
+    double imw;
     struct Raw { double p, q, r, s; };
-    __device__ __forceinline__ Raw fetch(long idx) const {
+    static constexpr int kModes = 2;       // mode 1: b0 == a0 (consecutive pairs of one row share the first orbital): 3 loads
+    __device__ __forceinline__ int mode() const { return b0 == a0 ? 1 : 0; }
+    template <int M> __device__ __forceinline__ Raw fetch(long idx) const {   // branch-free: the loads of a round issue back to back
         Raw w; w.p = __ldg(a0 + idx); w.q = __ldg(a1 + idx);
-        if (b0) { w.r = __ldg(b0 + idx); w.s = __ldg(b1 + idx); } else { w.r = 0.0; w.s = 0.0; }
+        w.r = (M == 1) ? w.p : __ldg(b0 + idx);
+        w.s = __ldg(b1 + idx);
         return w;
     }
-    __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2(w.p * w.q, w.r * w.s); }
+    __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2(w.p * w.q, imw * (w.r * w.s)); }
     // pull the operand planes [base, base + n) of the unit this CTA handles next into L2 (no registers held)
     __device__ __forceinline__ void prefetch_l2(long base, int n, int tid, int nthr) const {
         for (int e = tid * 16; e < n; e += nthr * 16) {          // one 128-byte line = 16 doubles
             asm volatile("prefetch.global.L2 [%0];" ::"l"(a0 + base + e));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(a1 + base + e));
-            if (b0) { asm volatile("prefetch.global.L2 [%0];" ::"l"(b0 + base + e)); asm volatile("prefetch.global.L2 [%0];" ::"l"(b1 + base + e)); }
+            if (b0 != a0) asm volatile("prefetch.global.L2 [%0];" ::"l"(b0 + base + e));
+            if (b1 != a1) asm volatile("prefetch.global.L2 [%0];" ::"l"(b1 + base + e));
         }
     }
 };
 struct BLoadPack2 {
     const double* s0; const double* s1; BatchLayout lay; long f; bool has_im; double scale;
     struct Raw { double p, q, r, s; };
-    __device__ __forceinline__ Raw fetch(long idx) const {
+    static constexpr int kModes = 1;
+    __device__ __forceinline__ int mode() const { return 0; }
+    template <int M> __device__ __forceinline__ Raw fetch(long idx) const {
         const long o0 = lay(f, idx);
         Raw w; w.p = s0[o0]; w.q = s1 ? s1[o0] : 0.0; w.r = 0.0; w.s = 0.0;
         if (has_im) { const long o1 = o0 + lay.next(); w.r = s0[o1]; if (s1) w.s = s1[o1]; }
@@ -88,8 +97,9 @@ __device__ __forceinline__ BLoadWork bind(const LoadWork& l, int b) { return BLo
 __device__ __forceinline__ BStoreWork bind(const StoreWork& s, int b) { return BStoreWork{s.work + (long)b * s.nr}; }
 __device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b) {
     const int2 p0 = l.pairs[2 * b];
-    BLoadPair r{l.phi + (long)p0.x * l.nr, l.phi + (long)p0.y * l.nr, nullptr, nullptr};
-    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr; r.b1 = l.phi + (long)p1.y * l.nr; }
+    BLoadPair r{l.phi + (long)p0.x * l.nr, l.phi + (long)p0.y * l.nr, nullptr, nullptr, 0.0};
+    r.b0 = r.a0; r.b1 = r.a1;
+    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr; r.b1 = l.phi + (long)p1.y * l.nr; r.imw = 1.0; }
     return r;
 }
 __device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b) { return BLoadPack2{l.src0, l.src1, l.lay, 2L * b, 2 * b + 1 < l.nfun, l.scale}; }
@@ -118,7 +128,7 @@ __device__ __forceinline__ void run_rounds(int tid, LoadF&& load, WorkF&& work) 
 template <class T, int R> struct RegBuf { T v[R]; };
 // registers per thread that still let MINB CTAs of NTHR threads share the 64 K register file (warp granularity 8 regs)
 template <int NTHR, int MINB> struct PlaneRegs {
-    static constexpr int warps = (NTHR + 31) / 32 * MINB;
+    static constexpr int warps = ((NTHR + 31) / 32 + 3) / 4 * 4 * MINB;    // warps are allocated four at a time
     static constexpr int raw = 65536 / (warps * 32) / 8 * 8;
     static constexpr int value = raw > 255 ? 255 : raw;
 };
@@ -154,23 +164,27 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
         }
         if constexpr (!INV) {
             // z stage 1 (radix R1z, twiddle after): global -> registers -> shared
-            run_rounds<NY * R2z, NTHR, DB1, RegBuf<Raw, R1z>>(tid,
-                [&](int t, RegBuf<Raw, R1z>& q) {
-                    const int y = t / R2z, i = t - y * R2z;
+            auto z1 = [&](auto mode_) {
+                constexpr int MD = decltype(mode_)::value;
+                run_rounds<NY * R2z, NTHR, DB1, RegBuf<Raw, R1z>>(tid,
+                    [&](int t, RegBuf<Raw, R1z>& q) {
+                        const int y = t / R2z, i = t - y * R2z;
 #pragma unroll
-                    for (int r = 0; r < R1z; ++r) q.v[r] = L.fetch(pbase + y * NZ + i + R2z * r);
-                },
-                [&](int t, const RegBuf<Raw, R1z>& q) {
-                    const int y = t / R2z, i = t - y * R2z;
-                    cplx x[R1z];
+                        for (int r = 0; r < R1z; ++r) q.v[r] = L.template fetch<MD>(pbase + y * NZ + i + R2z * r);
+                    },
+                    [&](int t, const RegBuf<Raw, R1z>& q) {
+                        const int y = t / R2z, i = t - y * R2z;
+                        cplx x[R1z];
 #pragma unroll
-                    for (int r = 0; r < R1z; ++r) x[r] = L.make(q.v[r]);
-                    Dft<R1z, false>::run(x);
-                    cplx* row = sm + y * PITCH;
-                    row[TZ::pad(i)] = x[0];
+                        for (int r = 0; r < R1z; ++r) x[r] = L.make(q.v[r]);
+                        Dft<R1z, false>::run(x);
+                        cplx* row = sm + y * PITCH;
+                        row[TZ::pad(i)] = x[0];
 #pragma unroll
-                    for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], wz[k]);
-                });
+                        for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], wz[k]);
+                    });
+            };
+            if (BL::kModes > 1 && L.mode() == 1) z1(IC<1>{}); else z1(IC<0>{});
             __syncthreads();
             // z stage 2 (radix R2z on blocks of R2z consecutive positions), in place
             run_rounds<NY * R1z, NTHR, DB2, RegBuf<cplx, R2z>>(tid,
@@ -225,7 +239,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                 [&](int t, RegBuf<Raw, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;
 #pragma unroll
-                    for (int i = 0; i < R2y; ++i) q.v[i] = L.fetch(pbase + (long)(k1 * R2y + i) * NZ + zp);
+                    for (int i = 0; i < R2y; ++i) q.v[i] = L.template fetch<0>(pbase + (long)(k1 * R2y + i) * NZ + zp);
                 },
                 [&](int t, const RegBuf<Raw, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;

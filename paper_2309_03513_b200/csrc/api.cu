@@ -71,16 +71,22 @@ static SArgs ypass_args(const tddft_ctx* c, int batch) {
     a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[1]; a.work = c->d_work; a.ktab = nullptr;
     return a;
 }
-static SArgs xpass_args(const tddft_ctx* c, int batch) {
+// Frequency-space work grids: full scrambled grids on the general path; on the fused path only the live (ky,kz)
+// columns of the transform's kind (plan.h: KIND_PROD = products of two sphere functions, KIND_SPHERE = sphere functions).
+enum { KIND_PROD = 0, KIND_SPHERE = 1 };
+static long work_stride(const tddft_ctx* c, int kind) { return c->fused ? (long)c->hp.n[0] * c->hp.ncols[kind] : c->hp.nr; }
+static SArgs xpass_args(const tddft_ctx* c, int batch, int kind) {
     const int* n = c->hp.n;
-    SArgs a{}; a.n = n[0]; a.stride = (long)n[1] * n[2]; a.inner = (long)n[1] * n[2]; a.nouter = 1; a.outer_stride = 0;
-    a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc;
+    const long inner = c->fused ? c->hp.ncols[kind] : (long)n[1] * n[2];
+    SArgs a{}; a.n = n[0]; a.stride = inner; a.inner = inner; a.nouter = 1; a.outer_stride = 0;
+    a.nr = work_stride(c, kind); a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc;
     return a;
 }
-static ZArgs zpass_args(const tddft_ctx* c, int batch) {
+static ZArgs zpass_args(const tddft_ctx* c, int batch, int kind) {
     const int* n = c->hp.n;
     ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.tw2 = c->d_tw[1]; a.work = c->d_work;
     a.lscale = 1.0; a.sscale = 1.0;
+    a.cmap = c->d_cmap[kind]; a.ncols = c->hp.ncols[kind]; a.wstride = work_stride(c, kind);
     return a;
 }
 
@@ -94,9 +100,9 @@ static int leg_forward_yz(tddft_ctx* c, int lkind, const ZArgs& z) {
     c->stats.kernel_launches += 2;
     return TDDFT_OK;
 }
-static int leg_x(tddft_ctx* c, int mode, int nb) {
-    if (c->fused) TD_CUDA(c, launch_xpass(mode, xpass_args(c, nb), c->stream));
-    else TD_CUDA(c, launch_spass(mode, xpass_args(c, nb), c->stream));
+static int leg_x(tddft_ctx* c, int mode, int nb, int kind) {
+    if (c->fused) TD_CUDA(c, launch_xpass(mode, xpass_args(c, nb, kind), c->stream));
+    else TD_CUDA(c, launch_spass(mode, xpass_args(c, nb, kind), c->stream));
     c->stats.kernel_launches += 1;
     return TDDFT_OK;
 }
@@ -115,10 +121,10 @@ static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pa
     for (long p0 = 0; p0 < npairs; p0 += 2L * c->fft_batch) {
         const int np = (int)std::min<long>(2L * c->fft_batch, npairs - p0);
         const int nb = (np + 1) / 2;
-        ZArgs z = zpass_args(c, nb);
+        ZArgs z = zpass_args(c, nb, KIND_PROD);
         z.phi = phi; z.pairs = d_pairs + p0; z.npairs = np;
         TD_RC(leg_forward_yz(c, ZL_PAIR, z));
-        TD_RC(leg_x(c, SM_CONV, nb));
+        TD_RC(leg_x(c, SM_CONV, nb, KIND_PROD));
         z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = p0; z.ftotal = npairs;
         TD_RC(leg_inverse_yz(c, z));
         c->stats.pair_ffts += np;
@@ -133,9 +139,9 @@ static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, d
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
         const int nb = (nf + 1) / 2;
-        TD_CUDA(c, launch_scatter_pack2(X, lay, f0, nfun, nb, c->d_idx_p, c->d_idx_m, c->d_work, nr, c->stream));
-        TD_RC(leg_x(c, SM_INV, nb));
-        ZArgs z = zpass_args(c, nb);
+        TD_CUDA(c, launch_scatter_pack2(X, lay, f0, nfun, nb, c->d_idx_p, c->d_idx_m, c->d_work, work_stride(c, KIND_SPHERE), c->stream));
+        TD_RC(leg_x(c, SM_INV, nb, KIND_SPHERE));
+        ZArgs z = zpass_args(c, nb, KIND_SPHERE);
         z.dst = dst; z.nfun = nf; z.sscale = scale; z.chunked = chunked; z.fbase = f0; z.ftotal = nfun;
         TD_RC(leg_inverse_yz(c, z));
         c->stats.kernel_launches += 1;
@@ -150,11 +156,11 @@ static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cpl
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
         const int nb = (nf + 1) / 2;
-        ZArgs z = zpass_args(c, nb);
+        ZArgs z = zpass_args(c, nb, KIND_SPHERE);
         z.src0 = src; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0; z.chunked = 1; z.fbase = f0; z.ftotal = nfun;
         TD_RC(leg_forward_yz(c, ZL_PACK2, z));
-        TD_RC(leg_x(c, SM_FWD, nb));
-        TD_CUDA(c, launch_gather_unpack2(c->d_work, nr, c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream));
+        TD_RC(leg_x(c, SM_FWD, nb, KIND_SPHERE));
+        TD_CUDA(c, launch_gather_unpack2(c->d_work, work_stride(c, KIND_SPHERE), c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream));
         c->stats.kernel_launches += 1;
     }
     return TDDFT_OK;
@@ -166,10 +172,10 @@ static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scal
     for (int f0 = 0; f0 < kc; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, kc - f0);
         const int nb = (nf + 1) / 2;
-        ZArgs z = zpass_args(c, nb);
+        ZArgs z = zpass_args(c, nb, KIND_PROD);
         z.src0 = d0; z.src1 = d1; z.nfun = nf; z.lscale = scale; z.chunked = 0; z.fbase = f0; z.ftotal = kc;
         TD_RC(leg_forward_yz(c, ZL_PACK2, z));
-        TD_RC(leg_x(c, SM_CONV, nb));
+        TD_RC(leg_x(c, SM_CONV, nb, KIND_PROD));
         z.dst = vh; z.sscale = 1.0;
         TD_RC(leg_inverse_yz(c, z));
     }
@@ -376,7 +382,7 @@ int tddft_enumerate_gvectors(const double* lattice, double ecut, long capacity, 
 
 int tddft_destroy(tddft_ctx* c) {
     if (!c) return TDDFT_OK;
-    cudaFree(c->d_idx_p); cudaFree(c->d_idx_m); cudaFree(c->d_kin); cudaFree(c->d_vc);
+    cudaFree(c->d_idx_p); cudaFree(c->d_idx_m); cudaFree(c->d_kin); cudaFree(c->d_vc); cudaFree(c->d_cmap[0]); cudaFree(c->d_cmap[1]);
     for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
     cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
@@ -442,16 +448,23 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_p, sizeof(int) * npwh));
         INIT_CUDA(cudaMalloc((void**)&c->d_idx_m, sizeof(int) * npwh));
         INIT_CUDA(cudaMalloc((void**)&c->d_kin, sizeof(double) * npwh));
-        INIT_CUDA(cudaMalloc((void**)&c->d_vc, sizeof(double) * nr));
+        const std::vector<double>& vc_h = c->fused ? c->hp.vc_c : c->hp.vc;
+        const std::vector<int>& idx_p_h = c->fused ? c->hp.idx_p_c : c->hp.idx_p;
+        const std::vector<int>& idx_m_h = c->fused ? c->hp.idx_m_c : c->hp.idx_m;
+        INIT_CUDA(cudaMalloc((void**)&c->d_vc, sizeof(double) * vc_h.size()));
+        if (c->fused) for (int k = 0; k < 2; ++k) {
+            INIT_CUDA(cudaMalloc((void**)&c->d_cmap[k], sizeof(int) * c->hp.colmap[k].size()));
+            INIT_CUDA(cudaMemcpy(c->d_cmap[k], c->hp.colmap[k].data(), sizeof(int) * c->hp.colmap[k].size(), cudaMemcpyHostToDevice));
+        }
         INIT_CUDA(cudaMalloc((void**)&c->d_work, sizeof(cplx) * nr * c->fft_batch));
         INIT_CUDA(cudaMalloc((void**)&c->d_zeros, 1024));
         INIT_CUDA(cudaMemset(c->d_zeros, 0, 1024));
         std::vector<double> kin(npwh);
         for (long g = 0; g < npwh; ++g) kin[g] = 0.5 * c->hp.g2[g];
-        INIT_CUDA(cudaMemcpy(c->d_idx_p, c->hp.idx_p.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
-        INIT_CUDA(cudaMemcpy(c->d_idx_m, c->hp.idx_m.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_idx_p, idx_p_h.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_idx_m, idx_m_h.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
         INIT_CUDA(cudaMemcpy(c->d_kin, kin.data(), sizeof(double) * npwh, cudaMemcpyHostToDevice));
-        INIT_CUDA(cudaMemcpy(c->d_vc, c->hp.vc.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
+        INIT_CUDA(cudaMemcpy(c->d_vc, vc_h.data(), sizeof(double) * vc_h.size(), cudaMemcpyHostToDevice));
         for (int a = 0; a < 3; ++a) {
             const int n = grid[a];
             std::vector<cplx> tw(n);

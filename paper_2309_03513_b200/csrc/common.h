@@ -36,6 +36,8 @@ struct ZArgs {
     // layout of the real function batches src0/src1/dst: function index fbase + (0..nfun-1) inside a batch of ftotal
     // functions; chunked = 0: [f][nr];  chunked = 1: [nr/32][ftotal][32] (CHUNK consecutive grid points per function)
     int chunked; long fbase; long ftotal;
+    // fused path only: pruned layout of the work grids (plan.h): column map, live columns, grid stride in `work`
+    const int* cmap; int ncols; long wstride;
 };
 constexpr int CHUNK = 32;
 inline long chunked_elems(long nfun, long nr) { return (nr + CHUNK - 1) / CHUNK * CHUNK * nfun; }

@@ -40,6 +40,7 @@ struct tddft_ctx {
     unsigned long long seed = 0;
     // device tables
     int *d_idx_p = nullptr, *d_idx_m = nullptr;
+    int* d_cmap[2] = {nullptr, nullptr};   // fused path: pruned column maps (plan.h), kind 0 = products, 1 = sphere functions
     double *d_kin = nullptr, *d_vc = nullptr, *d_eig[2] = {nullptr, nullptr};
     tddft::cplx* d_tw[3] = {nullptr, nullptr, nullptr};
     double* d_phi[2] = {nullptr, nullptr};

@@ -45,8 +45,8 @@ static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t 
 }
 template <int NY, int NZ, int NTHR, int MINB>
 static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
-    LoadWork lw{a.work, a.nr};
-    StoreWork sw{a.work, a.nr};
+    LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols};
+    StoreWorkC sw{a.work, a.wstride, a.cmap, a.ncols};
     const BatchLayout lay{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr};
     if (!inverse) {
         if (lkind == ZL_PAIR) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);

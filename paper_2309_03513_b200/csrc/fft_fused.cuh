@@ -38,72 +38,83 @@ template <int R1> __device__ __forceinline__ void load_twiddles(const cplx* __re
 // ---- bound load / store functors: per-unit state resolved once; loads are split into fetch (issue the global
 // loads, keep the raw operands in registers) and make (combine them), so that a round's loads can be issued one
 // round ahead of their use ---------------------------------------------------------------------------------------
-struct BLoadWork {
-    const cplx* g;
+// Work grids of the fused path are pruned (plan.h): element (x, column c) of packed grid b at b*gstride + x*ncols + c;
+// cmap maps a plane offset y*NZ + z to c, or -1 where the spectrum is identically zero (not stored, read as 0).
+struct LoadWorkC { const cplx* work; long gstride; const int* cmap; int ncols; };
+struct StoreWorkC { cplx* work; long gstride; const int* cmap; int ncols; };
+// Bound functors address one unit (packed grid b, plane x); `off` = y*NZ + z inside the plane.
+struct BLoadWorkC {
+    const cplx* g; const int* cmap;
     typedef cplx Raw;
     static constexpr int kModes = 1;
     __device__ __forceinline__ int mode() const { return 0; }
-    template <int M> __device__ __forceinline__ Raw fetch(long idx) const { return g[idx]; }
+    template <int M> __device__ __forceinline__ Raw fetch(int off) const {
+        const int c = __ldg(cmap + off);
+        return c >= 0 ? g[c] : make_double2(0.0, 0.0);
+    }
     __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
-    __device__ __forceinline__ void prefetch_l2(long, int, int, int) const {}
+    __device__ __forceinline__ void prefetch_l2(int, int, int) const {}
 };
-struct BStoreWork { cplx* g; __device__ __forceinline__ void operator()(long idx, cplx v) const { g[idx] = v; } };
+struct BStoreWorkC {
+    cplx* g; const int* cmap;
+    __device__ __forceinline__ void operator()(int off, cplx v) const { const int c = __ldg(cmap + off); if (c >= 0) g[c] = v; }
+};
 struct BLoadPair {
     const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = imw*b0*b1 (imw = 0 for the odd last pair, which reuses a0, a1)
     double imw;
     struct Raw { double p, q, r, s; };
     static constexpr int kModes = 2;       // mode 1: b0 == a0 (consecutive pairs of one row share the first orbital): 3 loads
     __device__ __forceinline__ int mode() const { return b0 == a0 ? 1 : 0; }
-    template <int M> __device__ __forceinline__ Raw fetch(long idx) const {   // branch-free: the loads of a round issue back to back
-        Raw w; w.p = __ldg(a0 + idx); w.q = __ldg(a1 + idx);
-        w.r = (M == 1) ? w.p : __ldg(b0 + idx);
-        w.s = __ldg(b1 + idx);
+    template <int M> __device__ __forceinline__ Raw fetch(int off) const {   // branch-free: the loads of a round issue back to back
+        Raw w; w.p = __ldg(a0 + off); w.q = __ldg(a1 + off);
+        w.r = (M == 1) ? w.p : __ldg(b0 + off);
+        w.s = __ldg(b1 + off);
         return w;
     }
     __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2(w.p * w.q, imw * (w.r * w.s)); }
-    // pull the operand planes [base, base + n) of the unit this CTA handles next into L2 (no registers held)
-    __device__ __forceinline__ void prefetch_l2(long base, int n, int tid, int nthr) const {
+    // pull the operand planes of the unit this CTA handles next into L2 (no registers held)
+    __device__ __forceinline__ void prefetch_l2(int n, int tid, int nthr) const {
         for (int e = tid * 16; e < n; e += nthr * 16) {          // one 128-byte line = 16 doubles
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(a0 + base + e));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(a1 + base + e));
-            if (b0 != a0) asm volatile("prefetch.global.L2 [%0];" ::"l"(b0 + base + e));
-            if (b1 != a1) asm volatile("prefetch.global.L2 [%0];" ::"l"(b1 + base + e));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a0 + e));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a1 + e));
+            if (b0 != a0) asm volatile("prefetch.global.L2 [%0];" ::"l"(b0 + e));
+            if (b1 != a1) asm volatile("prefetch.global.L2 [%0];" ::"l"(b1 + e));
         }
     }
 };
 struct BLoadPack2 {
-    const double* s0; const double* s1; BatchLayout lay; long f; bool has_im; double scale;
+    const double* s0; const double* s1; BatchLayout lay; long f; long pbase; bool has_im; double scale;
     struct Raw { double p, q, r, s; };
     static constexpr int kModes = 1;
     __device__ __forceinline__ int mode() const { return 0; }
-    template <int M> __device__ __forceinline__ Raw fetch(long idx) const {
-        const long o0 = lay(f, idx);
+    template <int M> __device__ __forceinline__ Raw fetch(int off) const {
+        const long o0 = lay(f, pbase + off);
         Raw w; w.p = s0[o0]; w.q = s1 ? s1[o0] : 0.0; w.r = 0.0; w.s = 0.0;
         if (has_im) { const long o1 = o0 + lay.next(); w.r = s0[o1]; if (s1) w.s = s1[o1]; }
         return w;
     }
     __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2((w.p + w.q) * scale, (w.r + w.s) * scale); }
-    __device__ __forceinline__ void prefetch_l2(long, int, int, int) const {}
+    __device__ __forceinline__ void prefetch_l2(int, int, int) const {}
 };
 struct BStoreSplit2 {
-    double* dst; BatchLayout lay; long f; bool has_im; double scale;
-    __device__ __forceinline__ void operator()(long idx, cplx v) const {
-        const long o0 = lay(f, idx);
+    double* dst; BatchLayout lay; long f; long pbase; bool has_im; double scale;
+    __device__ __forceinline__ void operator()(int off, cplx v) const {
+        const long o0 = lay(f, pbase + off);
         dst[o0] = v.x * scale;
         if (has_im) dst[o0 + lay.next()] = v.y * scale;
     }
 };
-__device__ __forceinline__ BLoadWork bind(const LoadWork& l, int b) { return BLoadWork{l.work + (long)b * l.nr}; }
-__device__ __forceinline__ BStoreWork bind(const StoreWork& s, int b) { return BStoreWork{s.work + (long)b * s.nr}; }
-__device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b) {
+__device__ __forceinline__ BLoadWorkC bind(const LoadWorkC& l, int b, int x, long) { return BLoadWorkC{l.work + (long)b * l.gstride + (long)x * l.ncols, l.cmap}; }
+__device__ __forceinline__ BStoreWorkC bind(const StoreWorkC& s, int b, int x, long) { return BStoreWorkC{s.work + (long)b * s.gstride + (long)x * s.ncols, s.cmap}; }
+__device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b, int, long pbase) {
     const int2 p0 = l.pairs[2 * b];
-    BLoadPair r{l.phi + (long)p0.x * l.nr, l.phi + (long)p0.y * l.nr, nullptr, nullptr, 0.0};
+    BLoadPair r{l.phi + (long)p0.x * l.nr + pbase, l.phi + (long)p0.y * l.nr + pbase, nullptr, nullptr, 0.0};
     r.b0 = r.a0; r.b1 = r.a1;
-    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr; r.b1 = l.phi + (long)p1.y * l.nr; r.imw = 1.0; }
+    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr + pbase; r.b1 = l.phi + (long)p1.y * l.nr + pbase; r.imw = 1.0; }
     return r;
 }
-__device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b) { return BLoadPack2{l.src0, l.src1, l.lay, 2L * b, 2 * b + 1 < l.nfun, l.scale}; }
-__device__ __forceinline__ BStoreSplit2 bind(const StoreSplit2& s, int b) { return BStoreSplit2{s.dst, s.lay, 2L * b, 2 * b + 1 < s.nfun, s.scale}; }
+__device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b, int, long pbase) { return BLoadPack2{l.src0, l.src1, l.lay, 2L * b, pbase, 2 * b + 1 < l.nfun, l.scale}; }
+__device__ __forceinline__ BStoreSplit2 bind(const StoreSplit2& s, int b, int, long pbase) { return BStoreSplit2{s.dst, s.lay, 2L * b, pbase, 2 * b + 1 < s.nfun, s.scale}; }
 
 // One phase = ITEMS butterflies spread over the CTA in rounds of NTHR.  The loads of round r+1 are issued before
 // round r is computed and stored (double-buffered registers), so memory latency overlaps the butterflies.
@@ -150,17 +161,16 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
 #pragma unroll
         for (int r = 0; r < R1y; ++r) wy[r] = wz[r];
     } else load_twiddles<R1y>(twy_g, tid % R2y, wy);
-    typedef decltype(bind(ld, 0)) BL;
+    typedef decltype(bind(ld, 0, 0, 0L)) BL;
     typedef typename BL::Raw Raw;
 
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
-        const int b = u / nx;
-        const long pbase = (long)(u - b * nx) * NY * NZ;
-        const BL L = bind(ld, b);
-        const auto S = bind(st, b);
+        const int b = u / nx, xpl = u - b * nx;
+        const BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
+        const auto S = bind(st, b, xpl, (long)xpl * NY * NZ);
         {   // operands of the unit this CTA takes next -> L2
             const int un = u + gridDim.x;
-            if (l2pf && un < nunits) { const int bn = un / nx; bind(ld, bn).prefetch_l2((long)(un - bn * nx) * NY * NZ, NY * NZ, tid, NTHR); }
+            if (l2pf && un < nunits) { const int bn = un / nx, xn = un - bn * nx; bind(ld, bn, xn, (long)xn * NY * NZ).prefetch_l2(NY * NZ, tid, NTHR); }
         }
         if constexpr (!INV) {
             // z stage 1 (radix R1z, twiddle after): global -> registers -> shared
@@ -170,7 +180,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                     [&](int t, RegBuf<Raw, R1z>& q) {
                         const int y = t / R2z, i = t - y * R2z;
 #pragma unroll
-                        for (int r = 0; r < R1z; ++r) q.v[r] = L.template fetch<MD>(pbase + y * NZ + i + R2z * r);
+                        for (int r = 0; r < R1z; ++r) q.v[r] = L.template fetch<MD>(y * NZ + i + R2z * r);
                     },
                     [&](int t, const RegBuf<Raw, R1z>& q) {
                         const int y = t / R2z, i = t - y * R2z;
@@ -231,7 +241,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                     const int k1 = t / NZ, zp = t - k1 * NZ;
                     Dft<R2y, false>::run(q.v);
 #pragma unroll
-                    for (int k = 0; k < R2y; ++k) S(pbase + (long)(k1 * R2y + k) * NZ + zp, q.v[k]);
+                    for (int k = 0; k < R2y; ++k) S((k1 * R2y + k) * NZ + zp, q.v[k]);
                 });
         } else {
             // y inverse stage R2y: global -> registers -> shared
@@ -239,7 +249,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                 [&](int t, RegBuf<Raw, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;
 #pragma unroll
-                    for (int i = 0; i < R2y; ++i) q.v[i] = L.template fetch<0>(pbase + (long)(k1 * R2y + i) * NZ + zp);
+                    for (int i = 0; i < R2y; ++i) q.v[i] = L.template fetch<0>((k1 * R2y + i) * NZ + zp);
                 },
                 [&](int t, const RegBuf<Raw, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;
@@ -300,7 +310,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                     for (int k = 1; k < R1z; ++k) q.v[k] = cmulc(q.v[k], wz[k]);
                     Dft<R1z, true>::run(q.v);
 #pragma unroll
-                    for (int r = 0; r < R1z; ++r) S(pbase + y * NZ + i + R2z * r, q.v[r]);
+                    for (int r = 0; r < R1z; ++r) S(y * NZ + i + R2z * r, q.v[r]);
                 });
         }
         __syncthreads();        // the plane buffer is reused by the next unit

@@ -115,6 +115,44 @@ const char* build_host_plan(const double* A, const int* grid, double ecut, HostP
         double k = 0.5 * (kval(j1, j2, j3) + kval((n1 - j1) % n1, (n2 - j2) % n2, (n3 - j3) % n3));
         hp->vc[flat(j1, j2, j3)] = k * inv_nr;
     }
+    // pruned layouts of the fused path (plan.h)
+    for (int kind = 0; kind < 2; ++kind) {
+        const double rad2 = (kind == 0 ? 4.0 : 1.0) * ecut * (1.0 + 1e-9);
+        const double gmax = std::sqrt(rad2);
+        int mb[3];
+        for (int i = 0; i < 3; ++i) {
+            double len = std::sqrt(A[3 * i] * A[3 * i] + A[3 * i + 1] * A[3 * i + 1] + A[3 * i + 2] * A[3 * i + 2]);
+            mb[i] = (int)std::floor(gmax * len / (2.0 * M_PI)) + 1;
+        }
+        std::vector<char> live((size_t)n2 * n3, 0);
+        for (int m1 = -mb[0]; m1 <= mb[0]; ++m1) for (int m2 = -mb[1]; m2 <= mb[1]; ++m2) for (int m3 = -mb[2]; m3 <= mb[2]; ++m3) {
+            double gx = m1 * hp->B[0] + m2 * hp->B[3] + m3 * hp->B[6];
+            double gy = m1 * hp->B[1] + m2 * hp->B[4] + m3 * hp->B[7];
+            double gz = m1 * hp->B[2] + m2 * hp->B[5] + m3 * hp->B[8];
+            if (gx * gx + gy * gy + gz * gz <= rad2) live[(size_t)hp->pos[1][wrap(m2, n2)] * n3 + hp->pos[2][wrap(m3, n3)]] = 1;
+        }
+        hp->colmap[kind].assign((size_t)n2 * n3, -1);
+        int nc = 0;
+        for (size_t o = 0; o < live.size(); ++o) if (live[o]) hp->colmap[kind][o] = nc++;
+        hp->ncols[kind] = nc;
+    }
+    {
+        const int nc0 = hp->ncols[0], nc1 = hp->ncols[1];
+        hp->vc_c.assign((size_t)n1 * nc0, 0.0);
+        for (int xp = 0; xp < n1; ++xp) for (long o = 0; o < (long)n2 * n3; ++o) {
+            const int cc = hp->colmap[0][o];
+            if (cc >= 0) hp->vc_c[(size_t)xp * nc0 + cc] = hp->vc[(size_t)xp * n2 * n3 + o];
+        }
+        hp->idx_p_c.resize(hp->npwh); hp->idx_m_c.resize(hp->npwh);
+        const long plane = (long)n2 * n3;
+        for (long g = 0; g < hp->npwh; ++g) {
+            const long ip = hp->idx_p[g], im = hp->idx_m[g];
+            const int cp = hp->colmap[1][ip % plane], cm = hp->colmap[1][im % plane];
+            if (cp < 0 || cm < 0) return "internal: sphere column outside the pruned layout";
+            hp->idx_p_c[g] = (int)((ip / plane) * nc1 + cp);
+            hp->idx_m_c[g] = (int)((im / plane) * nc1 + cm);
+        }
+    }
     return nullptr;
 }
 

@@ -2,6 +2,7 @@
 // Product path: every numerical step below is a kernel launch; the host only orchestrates.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "ctx.h"
@@ -116,16 +117,18 @@ static int leg_inverse_yz(tddft_ctx* c, const ZArgs& z) {
 #define TD_RC(call) do { int rc_ = (call); if (rc_) return rc_; } while (0)
 
 // tau_p = C[phi_i phi_j] for npairs pairs (device list), two pairs per complex grid
-static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, long npairs, double* tau, int chunked) {
+// d_slots (optional): tau slot of each pair; null = slot p for pair p.  batch_pairs <= 2*fft_batch pairs per launch.
+static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, const int* d_slots, long npairs, int batch_pairs, double* tau, int chunked) {
     const long nr = c->hp.nr;
-    for (long p0 = 0; p0 < npairs; p0 += 2L * c->fft_batch) {
-        const int np = (int)std::min<long>(2L * c->fft_batch, npairs - p0);
+    for (long p0 = 0; p0 < npairs; p0 += batch_pairs) {
+        const int np = (int)std::min<long>(batch_pairs, npairs - p0);
         const int nb = (np + 1) / 2;
         ZArgs z = zpass_args(c, nb, KIND_PROD);
         z.phi = phi; z.pairs = d_pairs + p0; z.npairs = np;
         TD_RC(leg_forward_yz(c, ZL_PAIR, z));
         TD_RC(leg_x(c, SM_CONV, nb, KIND_PROD));
-        z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = p0; z.ftotal = npairs;
+        z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = d_slots ? 0 : p0; z.ftotal = npairs;
+        z.slots = d_slots ? d_slots + p0 : nullptr;
         TD_RC(leg_inverse_yz(c, z));
         c->stats.pair_ffts += np;
     }
@@ -217,10 +220,26 @@ static int build_tiles(tddft_ctx* c, int spin, int T) {
     if (pt.T == T && pt.nocc == N && pt.d_pairs) return TDDFT_OK;
     if (pt.d_pairs) cudaFree(pt.d_pairs);
     if (pt.d_slot) cudaFree(pt.d_slot);
+    if (pt.d_pslot) cudaFree(pt.d_pslot);
     pt = PairTiles{};
     pt.T = T; pt.nocc = N;
+    // Processing order: sub-blocks of sbi rows x sbj columns (sbj even, sbi*sbj <= one launch of 2*fft_batch pairs), row-major
+    // inside a sub-block.  A launch then multiplies sbi + sbj orbital grids (L2 resident) instead of ~2*fft_batch, and the two
+    // pairs packed into one complex grid still share their first orbital.
+    {
+        const int cap = 2 * c->fft_batch;
+        double best = 1e300;
+        pt.sbi = 1; pt.sbj = std::max(2, cap & ~1);
+        for (int sj = 2; sj <= cap; sj += 2)
+            for (int si = 1; si * sj <= cap; ++si) {
+                const double fill = (double)(si * sj) / cap;
+                const double cost = (double)(si + sj) / (si * sj) / (fill * fill);
+                if (cost < best) { best = cost; pt.sbi = si; pt.sbj = sj; }
+            }
+        pt.batch_pairs = pt.sbi * pt.sbj;
+    }
     const int nb = (N + T - 1) / T;
-    std::vector<int2> pairs; std::vector<int> slot;
+    std::vector<int2> pairs; std::vector<int> slot, pslot;
     for (int bi = 0; bi < nb; ++bi)
         for (int bj = bi; bj < nb; ++bj) {
             TileInfo t{};
@@ -232,9 +251,17 @@ static int build_tiles(tddft_ctx* c, int spin, int T) {
                 for (int j = 0; j < t.tj; ++j) {
                     const int gi = t.i0 + i, gj = t.j0 + j;
                     if (gi > gj) continue;
-                    pairs.push_back(make_int2(gi, gj));
-                    s[(size_t)i * t.tj + j] = cnt++;
+                    s[(size_t)i * t.tj + j] = cnt++;     // tau slots stay row-major (the contraction's layout)
                 }
+            for (int si0 = 0; si0 < t.ti; si0 += pt.sbi)
+                for (int sj0 = 0; sj0 < t.tj; sj0 += pt.sbj)
+                    for (int i = si0; i < std::min(si0 + pt.sbi, t.ti); ++i)
+                        for (int j = sj0; j < std::min(sj0 + pt.sbj, t.tj); ++j) {
+                            const int gi = t.i0 + i, gj = t.j0 + j;
+                            if (gi > gj) continue;
+                            pairs.push_back(make_int2(gi, gj));
+                            pslot.push_back(s[(size_t)i * t.tj + j]);
+                        }
             if (bi == bj) for (int i = 0; i < t.ti; ++i) for (int j = 0; j < i; ++j) s[(size_t)i * t.tj + j] = s[(size_t)j * t.tj + i];
             t.npairs = cnt;
             slot.insert(slot.end(), s.begin(), s.end());
@@ -248,6 +275,8 @@ static int build_tiles(tddft_ctx* c, int spin, int T) {
         }
     TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * pairs.size()));
     TD_CUDA(c, cudaMalloc((void**)&pt.d_slot, sizeof(int) * slot.size()));
+    TD_CUDA(c, cudaMalloc((void**)&pt.d_pslot, sizeof(int) * pslot.size()));
+    TD_CUDA(c, cudaMemcpyAsync(pt.d_pslot, pslot.data(), sizeof(int) * pslot.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaMemcpyAsync(pt.d_pairs, pairs.data(), sizeof(int2) * pairs.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaMemcpyAsync(pt.d_slot, slot.data(), sizeof(int) * slot.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors go out of scope
@@ -286,14 +315,16 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     for (;;) {
         fixed = grid_b * (size_t)kc * ((size_t)sumocc + (size_t)maxocc + (hxc ? 2 * blocks.size() + 1 : 0))
               + sizeof(double) * project_scratch_doubles(c, maxocc, kc * maxocc, budget) + 4096;
-        T = std::min(std::min(maxocc, 128), c->pair_tile > 0 ? c->pair_tile : 128);
+        const int tcap = c->ct_full ? contract_full_max_tile() : 128;
+        T = std::min(std::min(maxocc, tcap), c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tcap);
         const int tmin = std::min(maxocc, 16);
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 8);
         if (fixed + grid_b * (size_t)T * T <= budget) break;
         if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
         kc = (kc + 1) / 2;
     }
-    if (T >= 32) T &= ~31;   // the contraction gives each warp 32 rows of a tile
+    if (c->ct_full) { const int nbk = (maxocc + T - 1) / T; T = (maxocc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
+    else if (T >= 32) T &= ~31;   // the row-block contraction gives each warp 32 rows of a tile
     int rc = ensure_arena(c, fixed + grid_b * (size_t)T * T);
     if (rc) return rc;
     char* p = c->arena;
@@ -342,9 +373,11 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
             if (c->alpha != 0.0) {
                 const PairTiles& pt = c->tiles[bl.src];
                 for (const TileInfo& t : pt.tiles) {
-                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, t.npairs, tau, 1); if (rc) return rc; }
+                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1); if (rc) return rc; }
                     StageTimer tm(c, ST_S5);
-                    if (t.slotT_off >= 0) TD_CUDA(c, launch_contract_dual(out, a[b], tau, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, nr, c->alpha, c->stream));
+                    if (c->ct_full) TD_CUDA(c, launch_contract_full(t.slotT_off < 0, out, a[b], tau, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc,
+                                                                   t.slotT_off < 0 ? (long)t.npairs : (long)t.ti * t.tj, nr, c->alpha, c->stream));
+                    else if (t.slotT_off >= 0) TD_CUDA(c, launch_contract_dual(out, a[b], tau, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, nr, c->alpha, c->stream));
                     else TD_CUDA(c, launch_contract_single(out, a[b], tau, pt.d_slot + t.slot_off, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, t.npairs, nr, c->alpha, c->stream));
                     c->stats.kernel_launches += (kcc + 15) / 16;
                 }
@@ -386,7 +419,7 @@ int tddft_destroy(tddft_ctx* c) {
     for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
     cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
-    for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); }
+    for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); cudaFree(c->tiles[s].d_pslot); }
     cudaGetLastError();
     delete c;
     return TDDFT_OK;
@@ -430,6 +463,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->fused = opt->fft_path == 0;
         } else c->fused = true;
         c->fused = c->fused && fused_supported(grid);
+        { const char* e = getenv("TDDFT_CT_FULL"); c->ct_full = !(e && atoi(e) == 0); }
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) {
             // latency-bound kernels: large launches beat L2 residency (measured); among the sizes up to 64 grids and 256 MB
@@ -552,7 +586,7 @@ int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs
     int2* d = nullptr;
     TD_CUDA(c, cudaMalloc((void**)&d, sizeof(int2) * n_pairs));
     cudaError_t e = cudaMemcpyAsync(d, pairs, sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, c->stream);
-    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, n_pairs, tau, 0) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
+    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, nullptr, n_pairs, 2 * c->fft_batch, tau, 0) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
     cudaStreamSynchronize(c->stream);
     cudaFree(d);
     return rc;

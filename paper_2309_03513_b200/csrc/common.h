@@ -33,6 +33,7 @@ struct ZArgs {
     double* dst;
     int nfun;
     double sscale;
+    const int* slots;      // optional (device, already offset to this launch): function index of packed function q is slots[q]
     // layout of the real function batches src0/src1/dst: function index fbase + (0..nfun-1) inside a batch of ftotal
     // functions; chunked = 0: [f][nr];  chunked = 1: [nr/32][ftotal][32] (CHUNK consecutive grid points per function)
     int chunked; long fbase; long ftotal;

@@ -14,8 +14,10 @@ struct TileInfo {
 struct PairTiles {
     int T = 0, nocc = 0;
     std::vector<TileInfo> tiles;
-    int2* d_pairs = nullptr;
+    int2* d_pairs = nullptr;   // pairs in processing order (sub-blocks of sbi x sbj, so a batch touches few orbitals)
+    int* d_pslot = nullptr;    // tau slot of each pair of d_pairs
     int* d_slot = nullptr;
+    int sbi = 0, sbj = 0, batch_pairs = 0;
     long max_pairs = 0;
 };
 
@@ -35,6 +37,7 @@ struct tddft_ctx {
     double workspace_gb = 0;
     int pair_tile = 0, fft_batch = 0;
     int num_sms = 148;
+    bool ct_full = true;             // S5 with the register-resident tile kernel (kernels.cu); TDDFT_CT_FULL=0 selects the row-block kernels
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off
     int dav_max_subspace = 0, dav_max_iter = 0; double dav_tol = 0; const double* dav_x0 = nullptr; int dav_nx0 = 0;
     unsigned long long seed = 0;

@@ -38,27 +38,94 @@ template <int R1> __device__ __forceinline__ void load_twiddles(const cplx* __re
 // ---- bound load / store functors: per-unit state resolved once; loads are split into fetch (issue the global
 // loads, keep the raw operands in registers) and make (combine them), so that a round's loads can be issued one
 // round ahead of their use ---------------------------------------------------------------------------------------
+// L2 eviction policy of the streams (work grids, tau, a(r) batches): evict_first keeps them from displacing the orbital planes
+// that the next launches read again.  hint = 0 gives the normal policy (same instructions, for A/B runs).
+__device__ __forceinline__ unsigned long long l2_policy(int hint) {
+    unsigned long long p;
+    if (hint) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_pol(cplx* p, cplx v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_pol(double* p, double v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ cplx ld_pol(const cplx* p, unsigned long long pol) {
+    cplx v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
 // Work grids of the fused path are pruned (plan.h): element (x, column c) of packed grid b at b*gstride + x*ncols + c;
 // cmap maps a plane offset y*NZ + z to c, or -1 where the spectrum is identically zero (not stored, read as 0).
-struct LoadWorkC { const cplx* work; long gstride; const int* cmap; int ncols; };
-struct StoreWorkC { cplx* work; long gstride; const int* cmap; int ncols; };
+struct LoadWorkC { const cplx* work; long gstride; const int* cmap; int ncols; int hint; };
+struct StoreWorkC { cplx* work; long gstride; const int* cmap; int ncols; int hint; };
 // Bound functors address one unit (packed grid b, plane x); `off` = y*NZ + z inside the plane.
 struct BLoadWorkC {
-    const cplx* g; const int* cmap;
+    const cplx* g; const int* cmap; int ncols; unsigned long long pol;
     typedef cplx Raw;
     static constexpr int kModes = 1;
     __device__ __forceinline__ int mode() const { return 0; }
     template <int M> __device__ __forceinline__ Raw fetch(int off) const {
         const int c = __ldg(cmap + off);
-        return c >= 0 ? g[c] : make_double2(0.0, 0.0);
+        return c >= 0 ? ld_pol(g + c, pol) : make_double2(0.0, 0.0);
     }
+    __device__ __forceinline__ Raw fetch_col(int c) const { return c >= 0 ? ld_pol(g + c, pol) : make_double2(0.0, 0.0); }
+    __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
+    __device__ __forceinline__ void prefetch_l2(int, int tid, int nthr) const {      // the compact plane is one contiguous run
+        for (int e = tid * 8; e < ncols; e += nthr * 8) asm volatile("prefetch.global.L2 [%0];" ::"l"(g + e));
+    }
+};
+struct BStoreWorkC {
+    cplx* g; const int* cmap; unsigned long long pol;
+    __device__ __forceinline__ void operator()(int off, cplx v) const { const int c = __ldg(cmap + off); if (c >= 0) st_pol(g + c, v, pol); }
+};
+// TMA-staged variant of LoadWorkC: the compact plane of the CTA's next unit (one contiguous run of ncols complex numbers)
+// is pulled into a shared-memory stage by one bulk async copy (cp.async.bulk, completion on an mbarrier) while the CTA
+// transforms the current unit, so the first butterflies read shared memory and no warp waits on global loads.
+struct LoadWorkT { const cplx* work; long gstride; const int* cmap; int ncols; int hint; };
+struct BLoadWorkT {
+    const cplx* stage; const int* cmap;
+    typedef cplx Raw;
+    static constexpr int kModes = 1;
+    __device__ __forceinline__ int mode() const { return 0; }
+    template <int M> __device__ __forceinline__ Raw fetch(int off) const {
+        const int c = __ldg(cmap + off);
+        return c >= 0 ? stage[c] : make_double2(0.0, 0.0);
+    }
+    __device__ __forceinline__ Raw fetch_col(int c) const { return c >= 0 ? stage[c] : make_double2(0.0, 0.0); }
     __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
     __device__ __forceinline__ void prefetch_l2(int, int, int) const {}
 };
-struct BStoreWorkC {
-    cplx* g; const int* cmap;
-    __device__ __forceinline__ void operator()(int off, cplx v) const { const int c = __ldg(cmap + off); if (c >= 0) g[c] = v; }
-};
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem, const void* gmem, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+template <class L> struct HasColMap { static constexpr bool value = false; };      // loads that go through the pruned column map
+template <> struct HasColMap<LoadWorkC> { static constexpr bool value = true; };
+template <> struct HasColMap<LoadWorkT> { static constexpr bool value = true; };
+template <class L> struct IsStaged { static constexpr bool value = false; };
+template <> struct IsStaged<LoadWorkT> { static constexpr bool value = true; };
 struct BLoadPair {
     const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = imw*b0*b1 (imw = 0 for the odd last pair, which reuses a0, a1)
     double imw;
@@ -82,30 +149,50 @@ struct BLoadPair {
         }
     }
 };
+// Real-function batches (BatchLayout) addressed from one unit: both the chunked layout [nr/32][function][32] and the plain
+// one [function][nr] (which is the chunked formula with a chunk stride of 32 elements) put point idx of function f at
+//   f_off + (idx >> 5) * cstride + (idx & 31),   f_off = f*32 (chunked) or f*nr (plain).
+// A bound functor keeps the byte address of (function, chunk of the plane's first point) and turns a plane offset into
+// one shift, one mask and one 32x32->64 multiply-add.
+struct UnitAddr {
+    unsigned r0;        // (first point of the plane) & 31
+    unsigned cs8;       // chunk stride in bytes
+    __device__ __forceinline__ size_t operator()(int off) const {
+        const unsigned i = r0 + (unsigned)off;
+        return (size_t)(i >> 5) * cs8 + (size_t)((i & 31u) * 8u);
+    }
+};
+__device__ __forceinline__ UnitAddr unit_addr(const BatchLayout& lay, long pbase) {
+    return UnitAddr{(unsigned)(pbase & 31), (unsigned)((lay.chunked ? lay.cstride : 32) * 8)};
+}
+__device__ __forceinline__ long fun_base(const BatchLayout& lay, long f, long pbase) {   // element offset of (f, chunk of pbase)
+    return lay.chunked ? (pbase >> 5) * lay.cstride + (lay.fbase + f) * CHUNK : (lay.fbase + f) * lay.nr + (pbase & ~31L);
+}
 struct BLoadPack2 {
-    const double* s0; const double* s1; BatchLayout lay; long f; long pbase; bool has_im; double scale;
+    const char *p0, *q0; long d1; UnitAddr ua; bool has_im; double scale;   // p0/q0: function 2b of src0/src1 (q0 may be null); d1: bytes to 2b+1
     struct Raw { double p, q, r, s; };
     static constexpr int kModes = 1;
     __device__ __forceinline__ int mode() const { return 0; }
     template <int M> __device__ __forceinline__ Raw fetch(int off) const {
-        const long o0 = lay(f, pbase + off);
-        Raw w; w.p = s0[o0]; w.q = s1 ? s1[o0] : 0.0; w.r = 0.0; w.s = 0.0;
-        if (has_im) { const long o1 = o0 + lay.next(); w.r = s0[o1]; if (s1) w.s = s1[o1]; }
+        const size_t o = ua(off);
+        Raw w; w.p = *(const double*)(p0 + o); w.q = q0 ? *(const double*)(q0 + o) : 0.0; w.r = 0.0; w.s = 0.0;
+        if (has_im) { w.r = *(const double*)(p0 + o + d1); if (q0) w.s = *(const double*)(q0 + o + d1); }
         return w;
     }
     __device__ __forceinline__ cplx make(const Raw& w) const { return make_double2((w.p + w.q) * scale, (w.r + w.s) * scale); }
     __device__ __forceinline__ void prefetch_l2(int, int, int) const {}
 };
 struct BStoreSplit2 {
-    double* dst; BatchLayout lay; long f; long pbase; bool has_im; double scale;
+    char* p0; long d1; UnitAddr ua; bool has_im; double scale; unsigned long long pol;
     __device__ __forceinline__ void operator()(int off, cplx v) const {
-        const long o0 = lay(f, pbase + off);
-        dst[o0] = v.x * scale;
-        if (has_im) dst[o0 + lay.next()] = v.y * scale;
+        char* q = p0 + ua(off);
+        st_pol((double*)q, v.x * scale, pol);
+        if (has_im) st_pol((double*)(q + d1), v.y * scale, pol);
     }
 };
-__device__ __forceinline__ BLoadWorkC bind(const LoadWorkC& l, int b, int x, long) { return BLoadWorkC{l.work + (long)b * l.gstride + (long)x * l.ncols, l.cmap}; }
-__device__ __forceinline__ BStoreWorkC bind(const StoreWorkC& s, int b, int x, long) { return BStoreWorkC{s.work + (long)b * s.gstride + (long)x * s.ncols, s.cmap}; }
+__device__ __forceinline__ BLoadWorkC bind(const LoadWorkC& l, int b, int x, long) { return BLoadWorkC{l.work + (long)b * l.gstride + (long)x * l.ncols, l.cmap, l.ncols, l2_policy(l.hint)}; }
+__device__ __forceinline__ BLoadWorkT bind(const LoadWorkT& l, int, int, long) { return BLoadWorkT{nullptr, l.cmap}; }
+__device__ __forceinline__ BStoreWorkC bind(const StoreWorkC& s, int b, int x, long) { return BStoreWorkC{s.work + (long)b * s.gstride + (long)x * s.ncols, s.cmap, l2_policy(s.hint)}; }
 __device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b, int, long pbase) {
     const int2 p0 = l.pairs[2 * b];
     BLoadPair r{l.phi + (long)p0.x * l.nr + pbase, l.phi + (long)p0.y * l.nr + pbase, nullptr, nullptr, 0.0};
@@ -113,8 +200,18 @@ __device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b, int, long pb
     if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr + pbase; r.b1 = l.phi + (long)p1.y * l.nr + pbase; r.imw = 1.0; }
     return r;
 }
-__device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b, int, long pbase) { return BLoadPack2{l.src0, l.src1, l.lay, 2L * b, pbase, 2 * b + 1 < l.nfun, l.scale}; }
-__device__ __forceinline__ BStoreSplit2 bind(const StoreSplit2& s, int b, int, long pbase) { return BStoreSplit2{s.dst, s.lay, 2L * b, pbase, 2 * b + 1 < s.nfun, s.scale}; }
+__device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b, int, long pbase) {
+    const long e0 = fun_base(l.lay, 2L * b, pbase);
+    return BLoadPack2{(const char*)(l.src0 + e0), l.src1 ? (const char*)(l.src1 + e0) : nullptr, l.lay.next() * 8, unit_addr(l.lay, pbase),
+                      2 * b + 1 < l.nfun, l.scale};
+}
+__device__ __forceinline__ BStoreSplit2 bind(const StoreSplit2& s, int b, int, long pbase) {
+    const bool has_im = 2 * b + 1 < s.nfun;
+    long f0 = 2L * b, f1 = f0 + 1;
+    if (s.slots) { f0 = s.slots[2 * b]; f1 = has_im ? s.slots[2 * b + 1] : f0; }
+    return BStoreSplit2{(char*)(s.dst + fun_base(s.lay, f0, pbase)), (f1 - f0) * s.lay.next() * 8, unit_addr(s.lay, pbase), has_im, s.scale,
+                        l2_policy(s.hint)};
+}
 
 // One phase = ITEMS butterflies spread over the CTA in rounds of NTHR.  The loads of round r+1 are issued before
 // round r is computed and stored (double-buffered registers), so memory latency overlaps the butterflies.
@@ -163,10 +260,46 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
     } else load_twiddles<R1y>(twy_g, tid % R2y, wy);
     typedef decltype(bind(ld, 0, 0, 0L)) BL;
     typedef typename BL::Raw Raw;
+    constexpr bool STAGED = IsStaged<Load>::value;
+    constexpr int NR0 = (NZ * R1y + NTHR - 1) / NTHR;   // rounds of the first inverse stage
+    int ccol[HasColMap<Load>::value ? NR0 : 1][R2y];
+    if constexpr (HasColMap<Load>::value) {
+#pragma unroll
+        for (int r = 0; r < NR0; ++r) {
+            const int t = tid + r * NTHR;
+            const int k1 = t / NZ, zp = t - k1 * NZ;
+#pragma unroll
+            for (int i = 0; i < R2y; ++i) ccol[r][i] = (t < NZ * R1y) ? __ldg(ld.cmap + (k1 * R2y + i) * NZ + zp) : -1;
+        }
+    }
+    static_assert(!STAGED || INV, "only the inverse kernel reads staged work grids");
+    cplx* stage = sm + NY * PITCH;                      // STAGED: [ncols] compact plane, then the mbarrier
+    unsigned long long* mbar = nullptr;
+    unsigned parity = 0;
+    if constexpr (STAGED) {
+        mbar = (unsigned long long*)(stage + ld.ncols);
+        if (tid == 0) {
+            mbar_init(mbar, 1);
+            if ((int)blockIdx.x < nunits) {
+                const int b0 = blockIdx.x / nx, x0 = blockIdx.x - b0 * nx;
+                mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
+                bulk_g2s(stage, ld.work + (long)b0 * ld.gstride + (long)x0 * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
+            }
+        }
+        __syncthreads();
+    }
 
+    // The CTAs of a launch start together and do identical work, so their load and compute phases stay aligned and the
+    // memory system sees bursts.  The second resident CTA of every SM (upper half of the grid) starts half a unit late.
+    {
+        const int stagger_ns = (l2pf >> 8) << 6;
+        if (stagger_ns > 0 && (int)blockIdx.x >= (int)(gridDim.x + 1) / 2) __nanosleep(stagger_ns);
+        l2pf &= 0xff;
+    }
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int b = u / nx, xpl = u - b * nx;
-        const BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
+        BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
+        if constexpr (STAGED) { L.stage = stage; mbar_wait(mbar, parity); parity ^= 1; }
         const auto S = bind(st, b, xpl, (long)xpl * NY * NZ);
         {   // operands of the unit this CTA takes next -> L2
             const int un = u + gridDim.x;
@@ -245,6 +378,22 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                 });
         } else {
             // y inverse stage R2y: global -> registers -> shared
+            if constexpr (HasColMap<Load>::value) {     // the thread's compact column indices are the same in every unit: registers
+#pragma unroll
+                for (int r = 0; r < NR0; ++r) {
+                    const int t = tid + r * NTHR;
+                    if (t < NZ * R1y) {
+                        const int k1 = t / NZ, zp = t - k1 * NZ;
+                        cplx x[R2y];
+#pragma unroll
+                        for (int i = 0; i < R2y; ++i) x[i] = L.fetch_col(ccol[r][i]);
+                        Dft<R2y, true>::run(x);
+                        cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
+#pragma unroll
+                        for (int i = 0; i < R2y; ++i) col[i * PITCH] = x[i];
+                    }
+                }
+            } else
             run_rounds<NZ * R1y, NTHR, DB1, RegBuf<Raw, R2y>>(tid,
                 [&](int t, RegBuf<Raw, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;
@@ -262,6 +411,14 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                     for (int i = 0; i < R2y; ++i) col[i * PITCH] = x[i];
                 });
             __syncthreads();
+            if constexpr (STAGED) {     // the stage is consumed: start the copy of this CTA's next unit behind the remaining stages
+                const int un = u + gridDim.x;
+                if (tid == 0 && un < nunits) {
+                    const int bn = un / nx, xn = un - bn * nx;
+                    mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
+                    bulk_g2s(stage, ld.work + (long)bn * ld.gstride + (long)xn * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
+                }
+            }
             // y inverse stage R1y (conjugate twiddle before the butterfly), in place
             run_rounds<NZ * R2y, NTHR, DB2, RegBuf<cplx, R1y>>(tid,
                 [&](int t, RegBuf<cplx, R1y>& q) {
@@ -329,16 +486,18 @@ template <int NX> struct XCfg {
     static constexpr int NTHR = G * XW;
     static constexpr size_t SMEM = sizeof(cplx) * NX * XW;
 };
+// Twiddles: the residue / block index g = tid / XW is the warp index (XW = 32), so every stage dispatches on g to a
+// body whose twiddles exp(-2 pi i g k / NX) are literals (mul_tw folds +-1, +-i and the octants): no twiddle registers
+// or loads, 3 CTAs per SM.  The barriers stay outside the per-warp bodies.
 template <int NX, int MODE>
-__global__ void __launch_bounds__(XCfg<NX>::NTHR, 2) xpass_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
-                                                                 const cplx* __restrict__ tw_g, const double* __restrict__ ktab) {
+__global__ void __launch_bounds__(XCfg<NX>::NTHR, 3) xpass_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
+                                                                 const cplx* __restrict__ tw_g, const double* __restrict__ ktab, int hint) {
+    const unsigned long long pol = l2_policy(hint);
     constexpr int R1 = XCfg<NX>::R1, R2 = XCfg<NX>::R2;
     extern __shared__ cplx sm[];
     const int tid = threadIdx.x, c = tid % XW, g = tid / XW;
     const long col = (long)blockIdx.x * XW + c;
     const bool live = col < inner;
-    cplx w[R1];
-    load_twiddles<R1>(tw_g, g < R2 ? g : 0, w);
     double kt[R2];
     if (MODE == SM_CONV) {
 #pragma unroll
@@ -347,22 +506,26 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, 2) xpass_kernel(cplx* __restri
     for (int b = blockIdx.y; b < batch; b += gridDim.y) {
         cplx* gcol = work + (long)b * nr + col;
         if (MODE == SM_FWD || MODE == SM_CONV) {
-            if (g < R2) {       // stage R1 forward: rows g + R2*r
-                cplx x[R1];
+            static_for<0, R2>([&](auto g_) {       // stage R1 forward of residue g: rows g + R2*r, twiddle after
+                constexpr int GI = decltype(g_)::value;
+                if (g == GI) {
+                    cplx x[R1];
 #pragma unroll
-                for (int r = 0; r < R1; ++r) x[r] = live ? gcol[(long)(g + R2 * r) * inner] : make_double2(0.0, 0.0);
-                Dft<R1, false>::run(x);
-                sm[g * XW + c] = x[0];
-#pragma unroll
-                for (int k = 1; k < R1; ++k) sm[(g + R2 * k) * XW + c] = cmul(x[k], w[k]);
-            }
+                    for (int r = 0; r < R1; ++r) x[r] = live ? ld_pol(gcol + (long)(GI + R2 * r) * inner, pol) : make_double2(0.0, 0.0);
+                    Dft<R1, false>::run(x);
+                    static_for<0, R1>([&](auto k_) {
+                        constexpr int K = decltype(k_)::value;
+                        sm[(GI + R2 * K) * XW + c] = mul_tw<false, NX, GI * K>(x[K]);
+                    });
+                }
+            });
             __syncthreads();
         }
         if (g < R1) {           // block g: rows g*R2 + i
             cplx x[R2];
             if (MODE == SM_INV) {
 #pragma unroll
-                for (int i = 0; i < R2; ++i) x[i] = live ? gcol[(long)(g * R2 + i) * inner] : make_double2(0.0, 0.0);
+                for (int i = 0; i < R2; ++i) x[i] = live ? ld_pol(gcol + (long)(g * R2 + i) * inner, pol) : make_double2(0.0, 0.0);
             } else {
 #pragma unroll
                 for (int i = 0; i < R2; ++i) x[i] = sm[(g * R2 + i) * XW + c];
@@ -371,7 +534,7 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, 2) xpass_kernel(cplx* __restri
             if (MODE == SM_FWD) {
                 if (live) {
 #pragma unroll
-                    for (int k = 0; k < R2; ++k) gcol[(long)(g * R2 + k) * inner] = x[k];
+                    for (int k = 0; k < R2; ++k) st_pol(gcol + (long)(g * R2 + k) * inner, x[k], pol);
                 }
             } else {
                 if (MODE == SM_CONV) {
@@ -385,17 +548,21 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, 2) xpass_kernel(cplx* __restri
         }
         if (MODE != SM_FWD) {
             __syncthreads();
-            if (g < R2) {       // stage R1 inverse: conjugate twiddle, butterfly, natural order out
-                cplx x[R1];
-                x[0] = sm[g * XW + c];
+            static_for<0, R2>([&](auto g_) {       // stage R1 inverse of residue g: conjugate twiddle, butterfly, natural order out
+                constexpr int GI = decltype(g_)::value;
+                if (g == GI) {
+                    cplx x[R1];
+                    static_for<0, R1>([&](auto k_) {
+                        constexpr int K = decltype(k_)::value;
+                        x[K] = mul_tw<true, NX, GI * K>(sm[(GI + R2 * K) * XW + c]);
+                    });
+                    Dft<R1, true>::run(x);
+                    if (live) {
 #pragma unroll
-                for (int k = 1; k < R1; ++k) x[k] = cmulc(sm[(g + R2 * k) * XW + c], w[k]);
-                Dft<R1, true>::run(x);
-                if (live) {
-#pragma unroll
-                    for (int r = 0; r < R1; ++r) gcol[(long)(g + R2 * r) * inner] = x[r];
+                        for (int r = 0; r < R1; ++r) st_pol(gcol + (long)(GI + R2 * r) * inner, x[r], pol);
+                    }
                 }
-            }
+            });
         }
         __syncthreads();        // the tile is reused by the next grid of the batch
     }

@@ -50,10 +50,11 @@ struct StoreWork {
 };
 struct StoreSplit2 {
     double* dst; int nfun; BatchLayout lay; double scale;
+    int hint;            // fused path: L2 eviction hint of the store stream (fft_fused.cuh)
+    const int* slots;    // optional: function index of packed function q is slots[q] instead of q (pair -> tau slot)
     __device__ __forceinline__ void operator()(int b, long idx, cplx v) const {
-        const long o0 = lay(2 * b, idx);
-        dst[o0] = v.x * scale;
-        if (2 * b + 1 < nfun) dst[o0 + lay.next()] = v.y * scale;
+        dst[lay(slots ? slots[2 * b] : 2 * b, idx)] = v.x * scale;
+        if (2 * b + 1 < nfun) dst[lay(slots ? slots[2 * b + 1] : 2 * b + 1, idx)] = v.y * scale;
     }
 };
 
@@ -154,7 +155,7 @@ cudaError_t zpass_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, c
         if (lkind == ZL_PACK2) return zpass_launch<N, false>(LoadPack2{a.src0, a.src1, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.lscale}, sw, a, s);
         return zpass_launch<N, false>(lw, sw, a, s);
     }
-    if (skind == ZS_SPLIT2) return zpass_launch<N, true>(lw, StoreSplit2{a.dst, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.sscale}, a, s);
+    if (skind == ZS_SPLIT2) return zpass_launch<N, true>(lw, StoreSplit2{a.dst, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.sscale, 0, a.slots}, a, s);
     return zpass_launch<N, true>(lw, sw, a, s);
 }
 template <int N>

@@ -36,6 +36,12 @@ cudaError_t launch_contract_single(double* out, const double* a, const double* t
                                    int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st);
 cudaError_t launch_contract_dual(double* out, const double* a, const double* tau, const double* zeros, int i0, int ti, int j0, int tj,
                                  int kc, long ftot, long nr, double alpha, cudaStream_t st);   // zeros: 256 B of device zeros
+// S5, register-resident variant: one launch does a whole tile with up to contract_full_max_tile() rows (any number of
+// columns); diag: ti == tj, same orbital block, tau packed upper-triangular (one direction, symmetric reads); else dense
+// slots i*tj + j and both directions.  stot = slots in the tau tile.
+int contract_full_max_tile();
+cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
+                                 long ftot, long stot, long nr, double alpha, cudaStream_t st);
 // S0: rho[r] = sum_v phi[v][r]^2 ; LDA kernel f_xc (Eq. 8; reading A5)
 cudaError_t launch_rho0(const double* phi, int nocc, long nr, double* rho, cudaStream_t st);
 cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double* fuu, double* fud,

@@ -22,6 +22,9 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the three S4 kernels per batch of 80 pairs at NV215, from the ncu --set full
+# capture summarised in profiles/r01d_ncu_s4.md (247.5 + 335.0 + 157.0 MB), per pair
+NCU_TRAFFIC_PER_PAIR = 739.5e6 / 80
 METRIC = "liouville_vector_applies_per_s"
 UNIT = "vector-applies/s"
 
@@ -274,13 +277,15 @@ def main():
     peak, peak_src = measured_peaks()
     s4_ms = stage_ms.get("ms_s4_pair_fft", 0.0)
     pairs_per_step = pair_ffts / max(args.steps, 1)
-    fft_batch = st["fft_batch"]
+    pb = st["pair_batch"]
     roofline = None
     if s4_ms > 0 and pair_ffts > 0:
         bytes_per_pair = 32.0 * nr                      # one HBM round trip per direction per pair density
         achieved = pair_ffts * bytes_per_pair / (s4_ms * 1e-3) / 1e9
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                    "traffic": None, "kernel": "S4 pair-FFT pipeline (%s, batches of %d pairs)" % ("plane_kernel fwd + xpass_kernel conv + plane_kernel inv" if st["fft_path"] == 0 else "5 general pass kernels", 2 * fft_batch),
+                    "traffic": NCU_TRAFFIC_PER_PAIR * pb if st["fft_path"] == 0 and args.config == 3 else None,
+                    "algorithmic_bytes": bytes_per_pair * pb, "units_per_launch": "%d pairs (one launch of each of the three kernels)" % pb,
+                    "kernel": "S4 pair-FFT pipeline (%s, batches of %d pairs)" % ("plane_kernel fwd + xpass_kernel conv + plane_kernel inv" if st["fft_path"] == 0 else "5 general pass kernels", pb),
                     "algorithmic_bytes_per_pair": bytes_per_pair, "peak_source": peak_src,
                     "share_of_step": s4_ms / max(stage_ms.get("ms_total", 1e-9), 1e-9)}
     cpu_baseline = None
@@ -292,7 +297,7 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": list(cfg["grid"]), "nocc": list(cfg["nocc"]), "nvec": nvec,
                    "mode": ["spin_conserving", "spin_flip_up_down", "spin_flip_down_up"][mode], "alpha": cfg["alpha"],
-                   "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": "images x%d" % world},
+                   "pair_tile": st["pair_tile"], "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": "images x%d" % world},
         "block_applies_per_s": value / nvec,
         "pair_ffts_per_s": (world * pair_ffts / (s4_ms * 1e-3)) if s4_ms > 0 else None,
         "pair_ffts_per_step": pairs_per_step,

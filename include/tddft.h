@@ -127,6 +127,8 @@ typedef struct {
   double ms_total, ms_s1_to_real, ms_s23_hxc, ms_s4_pair_fft, ms_s5_contract, ms_s6_to_sphere, ms_s8_project;
   int fft_batch; /* packed grids per FFT launch in use */
   int fft_path;  /* 0 = fused plane/x kernels, 1 = general pass kernels */
+  int pair_batch; /* orbital pairs per launch of the pair-FFT pipeline in the last apply (<= 2*fft_batch) */
+  int pair_tile;  /* tile edge of the last apply */
 } tddft_stats;
 int tddft_set_timing(tddft_ctx* ctx, int enabled); /* stage timing with CUDA events (adds synchronisation) */
 int tddft_get_stats(const tddft_ctx* ctx, tddft_stats* out);

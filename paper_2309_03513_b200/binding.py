@@ -37,7 +37,7 @@ class tddft_stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_longlong), ("pair_ffts", C.c_longlong), ("ms_total", C.c_double),
                 ("ms_s1_to_real", C.c_double), ("ms_s23_hxc", C.c_double), ("ms_s4_pair_fft", C.c_double),
                 ("ms_s5_contract", C.c_double), ("ms_s6_to_sphere", C.c_double), ("ms_s8_project", C.c_double),
-                ("fft_batch", C.c_int), ("fft_path", C.c_int)]
+                ("fft_batch", C.c_int), ("fft_path", C.c_int), ("pair_batch", C.c_int), ("pair_tile", C.c_int)]
 
 
 def load_library():

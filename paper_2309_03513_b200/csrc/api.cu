@@ -339,6 +339,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     double* O = carve(sizeof(double) * o_cap);
     double* tau = carve(grid_b * (size_t)T * T);
     for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src])); if (rc) return rc; }
+    c->last_pair_tile = T; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs;
 
     for (int k0 = 0; k0 < nvec; k0 += kc) {
         const int kcc = std::min(kc, nvec - k0);
@@ -576,6 +577,7 @@ int tddft_set_timing(tddft_ctx* c, int enabled) { if (!c) return TDDFT_EINVAL; c
 int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) {
     if (!c || !out) return TDDFT_EINVAL;
     *out = c->stats; out->fft_batch = c->fft_batch; out->fft_path = c->fused ? 0 : 1;
+    out->pair_batch = c->last_pair_batch; out->pair_tile = c->last_pair_tile;
     return TDDFT_OK;
 }
 

@@ -55,6 +55,7 @@ struct tddft_ctx {
     PairTiles tiles[2];
     // bookkeeping
     tddft_stats stats{};
+    int last_pair_batch = 0, last_pair_tile = 0;
     bool timing = false;
     std::vector<StageEvent> events;
     std::string err;

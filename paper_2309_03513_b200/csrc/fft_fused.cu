@@ -7,9 +7,9 @@
 namespace tddft {
 
 // (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
-// columns: NY, NZ, threads and CTAs per SM of the forward kernels, threads of the TMA-staged inverse kernel (one CTA per
-// SM, one butterfly per thread and stage; 0 = none), threads and CTAs per SM of the inverse kernel
-#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2, 648, 360, 2) X(48, 48, 96, 5, 0, 96, 5) X(24, 24, 96, 8, 0, 96, 8) X(18, 20, 96, 8, 0, 96, 8)
+// columns: NY, NZ, threads and CTAs per SM, threads of the TMA-staged inverse kernel (one CTA per SM, one butterfly per
+// thread and stage; 0 = none)
+#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2, 648) X(48, 48, 96, 5, 0) X(24, 24, 96, 8, 0) X(18, 20, 96, 8, 0)
 #define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
 
 static int plane_variant() {          // tuning switch TDDFT_VAR: bit 0 persistent grid, bit 3 L2 prefetch of the next unit's orbital planes, bit 4 of its work-grid plane, bit 5 evict-first L2 policy on the work-grid / tau / a(r) streams, bit 6 TMA-staged inverse plane kernel
@@ -41,9 +41,7 @@ static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t
     }
     const int var = plane_variant();
     const int grid = (var & 1) ? (nunits < resident ? nunits : resident) : nunits;
-    static int stagger = -1;         // TDDFT_STAGGER: start delay (ns) of the upper half of the grid, in units of 64 ns
-    if (stagger < 0) { const char* e = getenv("TDDFT_STAGGER"); stagger = e ? atoi(e) / 64 : 0; }
-    const int l2pf = (std::is_same<Load, LoadWorkC>::value ? ((var & 16) ? 1 : 0) : ((var & 8) ? 1 : 0)) | (grid >= resident ? stagger << 8 : 0);
+    const int l2pf = std::is_same<Load, LoadWorkC>::value ? ((var & 16) ? 1 : 0) : ((var & 8) ? 1 : 0);
     kern<<<grid, NTHR, smem, s>>>(ld, st, nx, nunits, l2pf, a.tw2, a.tw);
     return cudaGetLastError();
 }
@@ -52,7 +50,7 @@ static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t 
     // double-buffered rounds (DB1 / DB2 of plane_kernel) measured slower on B200 (register pressure): both off
     return plane_launch2<NY, NZ, NTHR, MINB, INV, false, false>(ld, st, a, s);
 }
-template <int NY, int NZ, int NTHR, int MINB, int TSTAGED, int NTHRI, int MINBI>
+template <int NY, int NZ, int NTHR, int MINB, int TSTAGED>
 static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
     const int hint = (plane_variant() & 32) ? 1 : 0;
     LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols, hint};
@@ -69,7 +67,6 @@ static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArg
         if (skind == ZS_SPLIT2 && (plane_variant() & 64) && need <= 227 * 1024)
             return plane_launch<NY, NZ, TSTAGED, 1, true>(LoadWorkT{a.work, a.wstride, a.cmap, a.ncols, hint}, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);
     }
-    if (skind == ZS_SPLIT2 && (plane_variant() & 128)) return plane_launch<NY, NZ, NTHRI, MINBI, true>(lw, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);
     if (skind == ZS_SPLIT2) return plane_launch<NY, NZ, NTHR, MINB, true>(lw, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);
     return cudaErrorInvalidValue;
 }
@@ -118,13 +115,13 @@ bool fused_supported(const int* n) {
 #define X(N) if (n[0] == N) px = true;
     TD_FOR_EACH_XLEN(X)
 #undef X
-#define X(NY, NZ, T, B, TS, TI, BI) if (n[1] == NY && n[2] == NZ) pl = true;
+#define X(NY, NZ, T, B, TS) if (n[1] == NY && n[2] == NZ) pl = true;
     TD_FOR_EACH_PLANE(X)
 #undef X
     return px && pl;
 }
 cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st) {
-#define X(NY, NZ, T, B, TS, TI, BI) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B, TS, TI, BI>(inverse, lkind, skind, a, st);
+#define X(NY, NZ, T, B, TS) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B, TS>(inverse, lkind, skind, a, st);
     TD_FOR_EACH_PLANE(X)
 #undef X
     return cudaErrorInvalidValue;

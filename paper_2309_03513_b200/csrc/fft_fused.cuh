@@ -289,13 +289,6 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
         __syncthreads();
     }
 
-    // The CTAs of a launch start together and do identical work, so their load and compute phases stay aligned and the
-    // memory system sees bursts.  The second resident CTA of every SM (upper half of the grid) starts half a unit late.
-    {
-        const int stagger_ns = (l2pf >> 8) << 6;
-        if (stagger_ns > 0 && (int)blockIdx.x >= (int)(gridDim.x + 1) / 2) __nanosleep(stagger_ns);
-        l2pf &= 0xff;
-    }
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int b = u / nx, xpl = u - b * nx;
         BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);

@@ -359,40 +359,47 @@ cudaError_t launch_contract_dual(double* out, const double* a, const double* tau
 // Row pitch 10 doubles and 108 rows per column make (row stride) = 8 mod 16 doubles, so both fragment patterns
 // (lanes over (i, j) for tau and over (j, i) for tau^T) spread over 8 distinct 8-byte banks: 4 wavefronts per load.
 // Results leave through shared memory so that every global access is a full 64-byte row.
-constexpr int FT_MT = 14;        // row tiles (8 rows) per warp
-constexpr int FT_IR = 108;       // rows per column in a stage = largest row block
-constexpr int FT_P = 8;          // grid points (= warps) per CTA
-constexpr int FT_PITCH = 10;     // doubles per shared-memory row
+// Tile shapes: MT row tiles of 8 per warp, IR rows per column in a stage (= largest row block; IR = 4 mod 8 for the bank pattern).
+// The smaller shape leaves registers for the compiler to run fragment loads ahead of the DMMAs.
+struct FullShapeL { static constexpr int MT = 14, IR = 108; };
+struct FullShapeS { static constexpr int MT = 11, IR = 92; static constexpr int TMAX = 88; };
+constexpr int FT_P = 4;          // grid points (= warps) per CTA: two CTAs per SM, so one CTA's prologue/epilogue hides behind the other's DMMAs
+constexpr int FT_PPR = FT_P / 2; // 16-byte pieces per shared-memory row
+constexpr int FT_PITCH = FT_P + 2;   // doubles per shared-memory row (rows stay 16-byte aligned)
 constexpr int FT_JS = 8;         // columns per stage
-template <int NK> struct FullCfg {
+template <int NK, class SH> struct FullCfg {
+    static constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
+    static_assert((FT_IR * FT_PITCH) % 16 == 8 && FT_PITCH % 2 == 0, "fragment bank pattern");
     static constexpr int KB = 8 * NK;                                   // trial vectors per launch
     static constexpr int ROWS = FT_JS * FT_IR + FT_JS * KB;             // rows of one stage
     static constexpr int STAGE = ROWS * FT_PITCH;                       // doubles
-    static constexpr int FLUSH = FT_JS * KB * FT_PITCH;                 // doubles
-    static constexpr size_t SMEM = sizeof(double) * (2 * STAGE + FLUSH);
+    static constexpr int FLUSH = FT_JS * KB * FT_PITCH;                 // doubles (two of them: products and prefetched out[J] rows)
+    static constexpr size_t SMEM = sizeof(double) * (2 * STAGE + 2 * FLUSH);
     static_assert(FT_MT * 8 * KB * FT_PITCH <= 2 * STAGE, "the epilogue stages the row block through the two stage buffers");
 };
-template <int NK, bool DIAG>
-__global__ void __launch_bounds__(32 * FT_P, 1)
+template <int NK, bool DIAG, class SH>
+__global__ void __launch_bounds__(32 * FT_P, 2)
 contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau,
                      int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
     extern __shared__ __align__(16) double sm[];
-    using C = FullCfg<NK>;
-    constexpr int KB = C::KB, IR = FT_IR, PITCH = FT_PITCH, JS = FT_JS;
-    constexpr int NTHR = 32 * FT_P;
+    using C = FullCfg<NK, SH>;
+    constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
+    constexpr int KB = C::KB, IR = FT_IR, PITCH = FT_PITCH, JS = FT_JS, PPR = FT_PPR;
+    constexpr int NTHR = 32 * FT_P, RSTEP = NTHR / PPR;     // rows covered by one pass of the CTA over 16-byte pieces
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, lr = lane >> 2, lc = lane & 3;
     const long chunk = blockIdx.x / (CHUNK / FT_P);
     const int pt0 = (int)(blockIdx.x % (CHUNK / FT_P)) * FT_P;
     const double* tau_c = tau + chunk * stot * CHUNK + pt0;
     const double* a_c = a + chunk * ftot * CHUNK + pt0;
     double* out_c = out + chunk * ftot * CHUNK + pt0;
-    const int piece2 = (tid & 3) * 2, rsub = tid >> 2;       // this thread's 16-byte piece of rows rsub, rsub + 64, ...
-    double* fl = sm + 2 * C::STAGE;
+    const int piece2 = (tid % PPR) * 2, rsub = tid / PPR;    // this thread's 16-byte piece of rows rsub, rsub + RSTEP, ...
+    double* fl = sm + 2 * C::STAGE;                          // products of the transposed direction, [8 j * KB][PITCH]
+    double* ojs = fl + C::FLUSH;                             // the out[J] rows they are subtracted from, prefetched by cp.async
 
     // ---- prologue: a[I] -> shared memory (coalesced) -> B fragments of the transposed product
     double breg[DIAG ? 1 : IR / 4][NK];
     if (!DIAG) {
-        for (int row = rsub; row < IR * KB; row += NTHR / 4) {
+        for (int row = rsub; row < IR * KB; row += RSTEP) {
             const int i = row / KB, kk = row - i * KB;
             double* dst = sm + row * PITCH + piece2;
             if (i < ti && kk < kn) cp_async16(dst, a_c + ((long)(i0 + i) * kc + kk) * CHUNK + piece2);
@@ -407,37 +414,38 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
             for (int n = 0; n < NK; ++n) breg[q][n] = sm[((q * 4 + lc) * KB + n * 8 + lr) * PITCH + w];
         __syncthreads();
     }
-    // Stage loader.  tau part: thread (w, lane) copies piece lane & 3 of column jj = lane >> 2, rows i = w, w + 8, ...: the
-    // source and destination advance by constants, so a copy costs a pointer increment.  a part: 8*KB rows, two per thread.
-    const int ljj = lane >> 2, lp2 = (lane & 3) * 2;
+    // Stage loader.  tau part: a group of 8*PPR lanes copies the pieces of the 8 columns of one row i; rows advance by a
+    // constant, so a copy costs a pointer increment.  a part: 8*KB rows spread over the CTA.
+    constexpr int LPR = 8 * PPR, RPW = 32 / LPR, ISTEP = FT_P * RPW;
+    const int ljj = (lane % LPR) / PPR, lp2 = (lane % PPR) * 2, li0 = w * RPW + lane / LPR;
     auto load_stage = [&](int buf, int js) {
         double* base = sm + buf * C::STAGE;
         const int col = js * JS + ljj;
-        double* dst = base + (ljj * IR + w) * PITCH + lp2;
+        double* dst = base + (ljj * IR + li0) * PITCH + lp2;
         if (col < tj) {
             if (DIAG) {
 #pragma unroll 2
-                for (int i = w; i < IR; i += FT_P, dst += FT_P * PITCH) {
+                for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH) {
                     if (i < ti) {
                         const int lo = min(i, col), hi = max(i, col);
                         cp_async16(dst, tau_c + ((long)lo * (2 * tj - lo + 1) / 2 + (hi - lo)) * CHUNK + lp2);
                     } else *(double2*)dst = make_double2(0.0, 0.0);
                 }
             } else {
-                const double* src = tau_c + ((long)w * tj + col) * CHUNK + lp2;
-                const long sstep = (long)FT_P * tj * CHUNK;
+                const double* src = tau_c + ((long)li0 * tj + col) * CHUNK + lp2;
+                const long sstep = (long)ISTEP * tj * CHUNK;
 #pragma unroll 2
-                for (int i = w; i < IR; i += FT_P, dst += FT_P * PITCH, src += sstep) {
+                for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH, src += sstep) {
                     if (i < ti) cp_async16(dst, src);
                     else *(double2*)dst = make_double2(0.0, 0.0);
                 }
             }
         } else {
-            for (int i = w; i < IR; i += FT_P, dst += FT_P * PITCH) *(double2*)dst = make_double2(0.0, 0.0);
+            for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH) *(double2*)dst = make_double2(0.0, 0.0);
         }
 #pragma unroll
-        for (int e = 0; e < (JS * KB * 4 + NTHR - 1) / NTHR; ++e) {
-            const int rr = rsub + e * (NTHR / 4);
+        for (int e = 0; e < (JS * KB + RSTEP - 1) / RSTEP; ++e) {
+            const int rr = rsub + e * RSTEP;
             if (rr < JS * KB) {
                 const int jj = rr / KB, kk = rr - jj * KB, cj = js * JS + jj;
                 double* d2 = base + (JS * IR + rr) * PITCH + piece2;
@@ -446,6 +454,7 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
             }
         }
     };
+    constexpr int NFL = (JS * KB + RSTEP - 1) / RSTEP;      // rows of out[J] per thread and stage
     double acc[FT_MT][NK][2];
 #pragma unroll
     for (int m = 0; m < FT_MT; ++m)
@@ -457,19 +466,17 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
     for (int js = 0; js < nst; ++js) {
         cp_async_wait<0>();
         __syncthreads();                 // stage js has landed for everyone; stage js-1 and its flush are consumed
+        if (!DIAG) {                     // rows of out[J] this thread updates after the transposed product: fetched behind the DMMAs
+#pragma unroll
+            for (int e = 0; e < NFL; ++e) {
+                const int row = rsub + e * RSTEP, jj = row / KB, kk = row - jj * KB, col = js * JS + jj;
+                if (row < JS * KB && col < tj && kk < kn) cp_async16(ojs + row * PITCH + piece2, out_c + ((long)(j0 + col) * kc + kk) * CHUNK + piece2);
+            }
+        }
+        cp_async_commit();
         if (js + 1 < nst) load_stage((js + 1) & 1, js + 1);
         cp_async_commit();
         const double* S = sm + (js & 1) * C::STAGE + w;
-        // rows of out[J] this thread updates after the transposed product (two 16-byte pieces), fetched behind the DMMAs
-        double2 oj[2]; double* ojp[2];
-        if (!DIAG) {
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int row = rsub + e * (NTHR / 4), jj = row / KB, kk = row - jj * KB, col = js * JS + jj;
-                ojp[e] = (row < JS * KB && col < tj && kk < kn) ? out_c + ((long)(j0 + col) * kc + kk) * CHUNK + piece2 : nullptr;
-                oj[e] = ojp[e] ? *(const double2*)ojp[e] : make_double2(0.0, 0.0);
-            }
-        }
         // direction 1: out[i][k] += sum_j tau[i][j] a[j][k]
 #pragma unroll
         for (int s = 0; s < JS / 4; ++s) {
@@ -499,18 +506,20 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
                 fl[(lr * KB + n * 8 + 2 * lc) * PITCH + w] = acc2[n][0];
                 fl[(lr * KB + n * 8 + 2 * lc + 1) * PITCH + w] = acc2[n][1];
             }
+            cp_async_wait<1>();          // this thread's out[J] pieces (the group before the next stage's copies)
             __syncthreads();
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                if (ojp[e]) {
-                    const int row = rsub + e * (NTHR / 4);
+            for (int e = 0; e < NFL; ++e) {
+                const int row = rsub + e * RSTEP, jj = row / KB, kk = row - jj * KB, col = js * JS + jj;
+                if (row < JS * KB && col < tj && kk < kn) {
                     const double2 d = *(const double2*)(fl + row * PITCH + piece2);
-                    *(double2*)ojp[e] = make_double2(fma(-alpha, d.x, oj[e].x), fma(-alpha, d.y, oj[e].y));
+                    const double2 o = *(const double2*)(ojs + row * PITCH + piece2);
+                    *(double2*)(out_c + ((long)(j0 + col) * kc + kk) * CHUNK + piece2) = make_double2(fma(-alpha, d.x, o.x), fma(-alpha, d.y, o.y));
                 }
             }
         }
     }
-    // ---- epilogue: out[I] -= alpha * acc through shared memory (64-byte rows)
+    // ---- epilogue: out[I] -= alpha * acc through shared memory (full rows)
     __syncthreads();
 #pragma unroll
     for (int m = 0; m < FT_MT; ++m)
@@ -520,50 +529,56 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
             sm[((m * 8 + lr) * KB + n * 8 + 2 * lc + 1) * PITCH + w] = acc[m][n][1];
         }
     __syncthreads();
-    constexpr int EB = 7;                // rows in flight per thread: the loads of a batch are issued before its stores
-    for (int row0 = rsub; row0 < ti * KB; row0 += EB * (NTHR / 4)) {
+    constexpr int EB = 14;               // rows in flight per thread: the loads of a batch are issued before its stores
+    for (int row0 = rsub; row0 < ti * KB; row0 += EB * RSTEP) {
         double2 o[EB]; double* p[EB];
 #pragma unroll
         for (int e = 0; e < EB; ++e) {
-            const int row = row0 + e * (NTHR / 4), i = row / KB, kk = row - i * KB;
+            const int row = row0 + e * RSTEP, i = row / KB, kk = row - i * KB;
             p[e] = (row < ti * KB && kk < kn) ? out_c + ((long)(i0 + i) * kc + kk) * CHUNK + piece2 : nullptr;
             o[e] = p[e] ? *(const double2*)p[e] : make_double2(0.0, 0.0);
         }
 #pragma unroll
         for (int e = 0; e < EB; ++e) {
             if (p[e]) {
-                const double2 d = *(const double2*)(sm + (row0 + e * (NTHR / 4)) * PITCH + piece2);
+                const double2 d = *(const double2*)(sm + (row0 + e * RSTEP) * PITCH + piece2);
                 *(double2*)p[e] = make_double2(fma(-alpha, d.x, o[e].x), fma(-alpha, d.y, o[e].y));
             }
         }
     }
 }
-template <int NK, bool DIAG>
+template <int NK, bool DIAG, class SH>
 static cudaError_t contract_full_launch(long nchunks, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj,
                                         int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    constexpr size_t smem = FullCfg<NK>::SMEM;
+    constexpr size_t smem = FullCfg<NK, SH>::SMEM;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(contract_full_kernel<NK, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(contract_full_kernel<NK, DIAG, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    contract_full_kernel<NK, DIAG><<<(unsigned)(nchunks * (CHUNK / FT_P)), 32 * FT_P, smem, st>>>(out, a, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
+    contract_full_kernel<NK, DIAG, SH><<<(unsigned)(nchunks * (CHUNK / FT_P)), 32 * FT_P, smem, st>>>(out, a, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
     return cudaGetLastError();
 }
-int contract_full_max_tile() { return FT_IR; }
+int contract_full_max_tile() { return FullShapeL::IR; }
+int contract_full_small_tile() { return FullShapeS::TMAX; }
+template <class SH>
+static cudaError_t contract_full_shape(bool diag, long nchunks, double* o, const double* ap, const double* tau, int i0, int ti, int j0, int tj,
+                                       int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
+    if (kn > 8) return diag ? contract_full_launch<2, true, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
+                            : contract_full_launch<2, false, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
+    return diag ? contract_full_launch<1, true, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
+                : contract_full_launch<1, false, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
+}
 cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
                                  long ftot, long stot, long nr, double alpha, cudaStream_t st) {
-    if (ti > FT_IR || tj < 1 || ti < 1 || (diag && ti != tj)) return cudaErrorInvalidValue;
+    if (ti > FullShapeL::IR || tj < 1 || ti < 1 || (diag && ti != tj)) return cudaErrorInvalidValue;
     const long nchunks = (nr + CHUNK - 1) / CHUNK;
     for (int kb = 0; kb < kc; kb += 16) {
         const int kn = kc - kb < 16 ? kc - kb : 16;
         double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
-        cudaError_t e;
-        if (kn > 8) e = diag ? contract_full_launch<2, true>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                             : contract_full_launch<2, false>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-        else e = diag ? contract_full_launch<1, true>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                      : contract_full_launch<1, false>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
+        cudaError_t e = ti <= FullShapeS::TMAX ? contract_full_shape<FullShapeS>(diag, nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
+                                               : contract_full_shape<FullShapeL>(diag, nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;

@@ -23,8 +23,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the three S4 kernels per batch of 80 pairs at NV215, from the ncu --set full
-# capture summarised in profiles/r01d_ncu_s4.md (247.5 + 335.0 + 157.0 MB), per pair
-NCU_TRAFFIC_PER_PAIR = 739.5e6 / 80
+# capture summarised in profiles/r01g_summary.md (179.5 + 245.4 + 335.5 MB), per pair
+NCU_TRAFFIC_PER_PAIR = 760.4e6 / 80
 METRIC = "liouville_vector_applies_per_s"
 UNIT = "vector-applies/s"
 
@@ -168,6 +168,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--pair-tile", type=int, default=0)
     ap.add_argument("--fft-batch", type=int, default=0)
+    ap.add_argument("--davidson", type=int, default=0, help="also run tddft_davidson for this many roots (not timed into `value`)")
+    ap.add_argument("--max-iter", type=int, default=0)
     args = ap.parse_args()
 
     from paper_2309_03513_b200 import inputs
@@ -204,6 +206,8 @@ def main():
         opts["pair_tile"] = args.pair_tile
     if args.fft_batch:
         opts["fft_batch"] = args.fft_batch
+    if args.max_iter:
+        opts["max_iter"] = args.max_iter
     ctx = b.tddft_init(cfg["lattice"], cfg["grid"], cfg["ecut"], cfg["nspin"], cfg["nocc"], d_psi[0],
                        d_psi[1] if cfg["nspin"] == 2 else None, inp["eig"][0],
                        inp["eig"][1] if cfg["nspin"] == 2 else None, cfg["alpha"], **opts)
@@ -269,6 +273,15 @@ def main():
         # sanity: host path equals device path
         assert torch.equal(AXp, dAX.cpu()), "host and device entry points disagree"
 
+    davidson = None
+    if args.davidson > 0 and rank == 0:      # SURVEY S9 on the same context: block Davidson for the lowest roots (reading A11)
+        del dX, dAX
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ev, iters, res = b.tddft_davidson(ctx, args.davidson, mode, allow_unconverged=True)
+        torch.cuda.synchronize()
+        davidson = {"nroots": args.davidson, "seconds": time.perf_counter() - t0, "iterations": int(iters),
+                    "eigenvalues_ha": [float(x) for x in ev], "residual_norms": [float(x) for x in res]}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -309,6 +322,8 @@ def main():
         "cpu_baseline": cpu_baseline,
         "workspace_gb": b.tddft_workspace_bytes(ctx) / 2 ** 30,
     }
+    if davidson:
+        line["davidson"] = davidson
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -214,6 +214,17 @@ size_t project_scratch_doubles(const tddft_ctx* c, int maxocc, int nrows, size_t
 }
 
 // ---- pair tiles -------------------------------------------------------------------------------------
+// sub-block of si rows x sj columns (sj even, si*sj <= cap pairs): few orbital grids per pair, launch well filled
+static void choose_subblock(int cap, int* si_out, int* sj_out) {
+    double best = 1e300;
+    *si_out = 1; *sj_out = std::max(2, cap & ~1);
+    for (int sj = 2; sj <= cap; sj += 2)
+        for (int si = 1; si * sj <= cap; ++si) {
+            const double fill = (double)(si * sj) / cap;
+            const double cost = (double)(si + sj) / (si * sj) / (fill * fill);
+            if (cost < best) { best = cost; *si_out = si; *sj_out = sj; }
+        }
+}
 static int build_tiles(tddft_ctx* c, int spin, int T) {
     PairTiles& pt = c->tiles[spin];
     const int N = c->nocc[spin];
@@ -226,18 +237,8 @@ static int build_tiles(tddft_ctx* c, int spin, int T) {
     // Processing order: sub-blocks of sbi rows x sbj columns (sbj even, sbi*sbj <= one launch of 2*fft_batch pairs), row-major
     // inside a sub-block.  A launch then multiplies sbi + sbj orbital grids (L2 resident) instead of ~2*fft_batch, and the two
     // pairs packed into one complex grid still share their first orbital.
-    {
-        const int cap = 2 * c->fft_batch;
-        double best = 1e300;
-        pt.sbi = 1; pt.sbj = std::max(2, cap & ~1);
-        for (int sj = 2; sj <= cap; sj += 2)
-            for (int si = 1; si * sj <= cap; ++si) {
-                const double fill = (double)(si * sj) / cap;
-                const double cost = (double)(si + sj) / (si * sj) / (fill * fill);
-                if (cost < best) { best = cost; pt.sbi = si; pt.sbj = sj; }
-            }
-        pt.batch_pairs = pt.sbi * pt.sbj;
-    }
+    choose_subblock(2 * c->fft_batch, &pt.sbi, &pt.sbj);
+    pt.batch_pairs = pt.sbi * pt.sbj;
     const int nb = (N + T - 1) / T;
     std::vector<int2> pairs; std::vector<int> slot, pslot;
     for (int bi = 0; bi < nb; ++bi)
@@ -467,13 +468,14 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         { const char* e = getenv("TDDFT_CT_FULL"); c->ct_full = !(e && atoi(e) == 0); }
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) {
-            // latency-bound kernels: large launches beat L2 residency (measured); among the sizes up to 64 grids and 256 MB
+            // latency-bound kernels: large launches beat L2 residency (measured); among the sizes up to 64 grids and 384 MB
             // take the one whose plane units (n1 per grid) fill whole waves of two CTAs per SM
-            const long cap = std::max<long>(1, std::min<long>(64, (256L << 20) / (16 * nr)));
+            const long cap = std::max<long>(1, std::min<long>(64, (384L << 20) / (16 * nr)));
             const long resident = 2L * c->num_sms;
             long bestb = cap; double beste = 0.0;
             for (long b = cap; b >= std::max<long>(1, cap / 2); --b) {
-                const long units = b * grid[0], waves = (units + resident - 1) / resident;
+                int si, sj; choose_subblock((int)(2 * b), &si, &sj);
+                const long units = (long)(si * sj + 1) / 2 * grid[0], waves = (units + resident - 1) / resident;   // grids a pair launch really holds
                 const double e = (double)units / (double)(waves * resident);
                 if (e > beste + 0.01) { beste = e; bestb = b; }
             }

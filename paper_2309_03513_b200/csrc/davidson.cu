@@ -6,6 +6,8 @@
 // The host only decides convergence from the residual norms.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <vector>
 #include "ctx.h"
 
@@ -228,8 +230,9 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     }
     for (int i = 0; i < nstart; ++i) {
         if (c->dav_x0 && c->dav_nx0 > 0) DV_TRY(cudaMemcpyAsync(T, c->dav_x0 + (long)i * n2, sizeof(double) * n2, cudaMemcpyDeviceToDevice, st));
-        else {   // unit vector on the i-th smallest diagonal element |G|^2/2 - eps_v plus 1e-3 seeded noise (reading A11)
-            random_start_kernel<<<eb, 256, 0, st>>>((cplx*)T, L, npwh, c->seed * 0x100000001B3ull + 0x51ED27ull + (unsigned long long)i * (unsigned long long)(2 * L + 2), 1e-3, guess[i]);
+        else {   // unit vector on the i-th smallest diagonal element |G|^2/2 - eps_v plus seeded noise of 2-norm ~1e-3 (reading A11):
+                 // the amplitude per component scales with 1/sqrt(2L), or the noise would swamp the unit vector at L ~ 10^7
+            random_start_kernel<<<eb, 256, 0, st>>>((cplx*)T, L, npwh, c->seed * 0x100000001B3ull + 0x51ED27ull + (unsigned long long)i * (unsigned long long)(2 * L + 2), 1e-3 / sqrt(2.0 * (double)L), guess[i]);
             DV_TRY(cudaGetLastError()); ++launches;
         }
         DV_RC(project_vec(T));
@@ -239,6 +242,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     if (m == 0) { cleanup(); return set_err(c, TDDFT_EINVAL, "davidson: start vectors vanish after projection"); }
 
     std::vector<double> h_theta(max_sub), h_res(nroots, 0.0), h_r2(nroots * nroots);
+    const bool trace = getenv("TDDFT_DAV_TRACE") != nullptr;     // one line per iteration on stderr
     int it = 0, status = TDDFT_ENOTCONVERGED, nr = 0;
     for (it = 1; it <= max_iter; ++it) {
         if (mw < m) {      // W = A V for the new columns
@@ -270,6 +274,13 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
         DV_TRY(cudaStreamSynchronize(st));
         bool all = (nr == nroots);
         for (int i = 0; i < nr; ++i) { h_res[i] = std::sqrt(std::max(h_r2[(size_t)i * nr + i], 0.0)); if (h_res[i] > tol) all = false; }
+        if (trace) {
+            fprintf(stderr, "davidson it %d m %d theta", it, m);
+            for (int i = 0; i < nr; ++i) fprintf(stderr, " %.6e", h_theta[i]);
+            fprintf(stderr, " res");
+            for (int i = 0; i < nr; ++i) fprintf(stderr, " %.2e", h_res[i]);
+            fprintf(stderr, "\n");
+        }
         if (all) { status = TDDFT_OK; break; }
         if (it == max_iter) break;
         // restart when the new vectors would not fit: keep the Ritz vectors and their images

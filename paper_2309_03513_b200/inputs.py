@@ -136,11 +136,11 @@ def make_trial_block(cfg, inputs, nvec, mode):
 
 def diagonal_guess(rng, diag, npwh, nvec, noise=1e-3):
     """Davidson start vectors: unit vectors on the nvec smallest entries of `diag` (the caller's
-    |G|^2/2 - eps_v per element of a trial vector) plus a little seeded noise; Im c(G=0) = 0."""
+    |G|^2/2 - eps_v per element of a trial vector) plus seeded noise of 2-norm ~`noise`; Im c(G=0) = 0."""
     diag = np.asarray(diag)
     order = np.argsort(diag, kind="stable")[:nvec]
     L = diag.size
-    x0 = noise * (rng.standard_normal((nvec, L)) + 1j * rng.standard_normal((nvec, L)))
+    x0 = noise / np.sqrt(2.0 * L) * (rng.standard_normal((nvec, L)) + 1j * rng.standard_normal((nvec, L)))
     for i, e in enumerate(order):
         x0[i, e] += 1.0
     x0.reshape(nvec, -1, npwh)[:, :, 0] = x0.reshape(nvec, -1, npwh)[:, :, 0].real

@@ -40,6 +40,19 @@ def test_options_struct_layout_matches_header(binding):
     assert names == [f[0] for f in binding.tddft_options._fields_]
 
 
+def test_stats_struct_layout_matches_header(binding):
+    hdr = open(os.path.join(ROOT, "include", "tddft.h")).read()
+    body = hdr[hdr.index("typedef struct {", hdr.index("Counters of the last tddft_apply_liouville call")):]
+    body = body[:body.index("} tddft_stats;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.replace("typedef struct {", "").split(";"):
+        decl = decl.strip()
+        if decl:
+            names += [n.strip() for n in re.sub(r"^(long long|double|int)\s+", "", decl).split(",")]
+    assert names == [f[0] for f in binding.tddft_stats._fields_]
+
+
 HEX = [[36.9, 0, 0], [-18.45, 36.9 * math.sqrt(3) / 2, 0], [0, 0, 19.5]]
 
 

@@ -108,7 +108,9 @@ int tddft_workspace_bytes(const tddft_ctx* ctx, long long* bytes);
  * X read-only, AX must not alias X.  The operator projects its output only (Eqs. 3-6 apply P_c on the left). */
 int tddft_apply_liouville(tddft_ctx* ctx, const double* X, double* AX, int nvec, int mode);
 
-/* Same with HOST buffers: copies X to the device, applies, copies AX back, synchronises. */
+/* Same with HOST buffers (pinned memory recommended): copies X to the device, applies, copies AX back, synchronises.
+ * The copies run on a stream of their own, one spin block at a time, so that a finished block of AX travels back while
+ * the next block is still being computed.  Returns after both streams have drained. */
 int tddft_apply_liouville_host(tddft_ctx* ctx, const double* X_host, double* AX_host, int nvec, int mode);
 
 /* Lowest nroots of A by block Davidson (reading A11).

@@ -348,6 +348,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
         for (size_t b = 0; b < blocks.size(); ++b) {
             const int no = c->nocc[blocks[b].src];
             FunLayout lay{L, blocks[b].off, npwh, kcc, k0};
+            if (c->overlap_copies) TD_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_x_ready[b], 0));     // this block of X has arrived
             { StageTimer t(c, ST_S1); rc = to_real_space(c, X, lay, no * kcc, a[b], 1); if (rc) return rc; }
             if (hxc) { StageTimer t(c, ST_S23); TD_CUDA(c, launch_drho(c->d_phi[blocks[b].src], a[b], no, kcc, nr, drho[b], c->stream)); c->stats.kernel_launches += (kcc + 3) / 4; }
         }
@@ -390,6 +391,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
             // S8: conduction-band projector of the target spin
             { StageTimer t(c, ST_S8);
               rc = project_rows(c, bl.tgt, (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, O, o_cap); if (rc) return rc; }
+            if (c->overlap_copies) TD_CUDA(c, cudaEventRecord(c->ev_ax_done[b], c->stream));               // this block of AX is final
         }
     }
     collect_timing(c);
@@ -421,6 +423,8 @@ int tddft_destroy(tddft_ctx* c) {
     for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
     cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (int i = 0; i < 2; ++i) { if (c->ev_x_ready[i]) cudaEventDestroy(c->ev_x_ready[i]); if (c->ev_ax_done[i]) cudaEventDestroy(c->ev_ax_done[i]); }
     for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); cudaFree(c->tiles[s].d_pslot); }
     cudaGetLastError();
     delete c;
@@ -566,11 +570,47 @@ int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int 
     if (cudaMalloc((void**)&dX, bytes) != cudaSuccess || cudaMalloc((void**)&dAX, bytes) != cudaSuccess) {
         cudaGetLastError(); cudaFree(dX); return set_err(c, TDDFT_ENOMEM, "apply_host: device allocation failed");
     }
+    // The spin blocks of a spin-conserving vector are processed one after the other (apply_liouville_dev), so block 1 of X
+    // is copied in while block 0 is computed and block 0 of AX is copied out while block 1 is computed: the copies run on
+    // their own stream as 2-D copies (nvec rows of one block, pitch = one trial vector), ordered by events.
+    const int nblk = (mode == TDDFT_SPIN_CONSERVING) ? c->nspin : 1;
     int rc = TDDFT_OK;
-    if (cudaMemcpyAsync(dX, Xh, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: H2D copy failed");
-    if (!rc) rc = tddft_apply_liouville(c, dX, dAX, nvec, mode);
-    if (!rc && cudaMemcpyAsync(AXh, dAX, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: D2H copy failed");
+    if (!c->copy_stream) {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: stream creation failed");
+        for (int i = 0; i < 2 && !rc; ++i)
+            if (cudaEventCreateWithFlags(&c->ev_x_ready[i], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_ax_done[i], cudaEventDisableTiming) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: event creation failed");
+    }
+    const size_t pitch = sizeof(cplx) * (size_t)L;
+    size_t boff[2] = {0, 0}, bw[2] = {pitch, 0};
+    if (nblk == 2) { bw[0] = sizeof(cplx) * (size_t)c->nocc[0] * c->hp.npwh; boff[1] = bw[0]; bw[1] = pitch - bw[0]; }
+    cudaEvent_t start = nullptr;
+    if (!rc && cudaEventCreateWithFlags(&start, cudaEventDisableTiming) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: event creation failed");
+    if (!rc) {      // the copies start where the caller's stream stands now
+        cudaEventRecord(start, c->stream);
+        cudaStreamWaitEvent(c->copy_stream, start, 0);
+        for (int b = 0; b < nblk && !rc; ++b) {
+            if (cudaMemcpy2DAsync((char*)dX + boff[b], pitch, (const char*)Xh + boff[b], pitch, bw[b], nvec, cudaMemcpyHostToDevice, c->copy_stream) != cudaSuccess ||
+                cudaEventRecord(c->ev_x_ready[b], c->copy_stream) != cudaSuccess) rc = set_err(c, TDDFT_ECUDA, "apply_host: H2D copy failed");
+        }
+    }
+    if (!rc) {
+        c->overlap_copies = true;
+        rc = tddft_apply_liouville(c, dX, dAX, nvec, mode);
+        c->overlap_copies = false;
+    }
+    if (!rc) {
+        for (int b = 0; b < nblk && !rc; ++b) {
+            if (cudaStreamWaitEvent(c->copy_stream, c->ev_ax_done[b], 0) != cudaSuccess ||
+                cudaMemcpy2DAsync((char*)AXh + boff[b], pitch, (const char*)dAX + boff[b], pitch, bw[b], nvec, cudaMemcpyDeviceToHost, c->copy_stream) != cudaSuccess)
+                rc = set_err(c, TDDFT_ECUDA, "apply_host: D2H copy failed");
+        }
+        // the caller's stream continues after the last copy
+        if (!rc && (cudaEventRecord(start, c->copy_stream) != cudaSuccess || cudaStreamWaitEvent(c->stream, start, 0) != cudaSuccess)) rc = set_err(c, TDDFT_ECUDA, "apply_host: stream join failed");
+    }
+    if (cudaStreamSynchronize(c->copy_stream) != cudaSuccess && !rc) rc = set_err(c, TDDFT_ECUDA, "apply_host: copy stream failed");
     if (cudaStreamSynchronize(c->stream) != cudaSuccess && !rc) rc = set_err(c, TDDFT_ECUDA, "apply_host: stream failed");
+    if (start) cudaEventDestroy(start);
     cudaFree(dX); cudaFree(dAX);
     return rc;
 }

@@ -53,6 +53,10 @@ struct tddft_ctx {
     // per-call workspace arena
     char* arena = nullptr; size_t arena_bytes = 0;
     PairTiles tiles[2];
+    // host-buffer entry point: copies run on their own stream, block by block, behind the kernels (api.cu)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_x_ready[2] = {nullptr, nullptr}, ev_ax_done[2] = {nullptr, nullptr};
+    bool overlap_copies = false;     // set only while tddft_apply_liouville_host drives an apply
     // bookkeeping
     tddft_stats stats{};
     int last_pair_batch = 0, last_pair_tile = 0;

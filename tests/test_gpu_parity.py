@@ -82,3 +82,23 @@ def test_tiling_and_k_chunking_do_not_change_the_result():
     assert rel_fro(tiled.gpu_apply(X, 0), ref) < TOL
     capped = Case(TRI, (12, 10, 9), 6.0, 2, (7, 5), 0.3, seed=105, oracle=False, workspace_gb=0.0007)
     assert rel_fro(capped.gpu_apply(X, 0), ref) < TOL
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_host_buffer_entry_point_equals_device_path(mode):
+    # tddft_apply_liouville_host copies block by block on its own stream behind the kernels: same bits as the device call,
+    # from pageable numpy buffers and from pinned ones, and repeatable
+    import torch
+    from paper_2309_03513_b200 import binding as b
+    case = Case(TRI, (12, 18, 20), 6.0, 2, (5, 4), 0.3, seed=106)
+    X = case.trial(3, mode)
+    ref = case.gpu_apply(X, mode)
+    assert rel_fro(ref, case.oracle.apply(X, mode)) < TOL
+    out = np.empty_like(X)
+    b.tddft_apply_liouville_host(case.ctx(), np.ascontiguousarray(X), out, 3, mode)
+    assert np.array_equal(out, ref)
+    Xp = torch.from_numpy(X).pin_memory(); AXp = torch.empty_like(Xp).pin_memory()
+    for _ in range(2):
+        AXp.zero_()
+        b.tddft_apply_liouville_host(case.ctx(), Xp, AXp, 3, mode)
+        assert np.array_equal(AXp.numpy(), ref)

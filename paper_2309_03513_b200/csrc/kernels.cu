@@ -367,6 +367,7 @@ constexpr int FT_P = 4;          // grid points (= warps) per CTA: two CTAs per 
 constexpr int FT_PPR = FT_P / 2; // 16-byte pieces per shared-memory row
 constexpr int FT_PITCH = FT_P + 2;   // doubles per shared-memory row (rows stay 16-byte aligned)
 constexpr int FT_JS = 8;         // columns per stage
+constexpr int FT_PF = 3;         // A fragments in flight ahead of the DMMAs (5 measured no better, copies interleaved with the DMMAs worse)
 template <int NK, class SH> struct FullCfg {
     static constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
     static_assert((FT_IR * FT_PITCH) % 16 == 8 && FT_PITCH % 2 == 0, "fragment bank pattern");
@@ -483,9 +484,16 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
             double bf[NK];
 #pragma unroll
             for (int n = 0; n < NK; ++n) bf[n] = S[(JS * IR + (s * 4 + lc) * KB + n * 8 + lr) * PITCH];
+            // the A fragments run FT_PF tiles ahead of the DMMAs that use them (explicit rotation: the compiler does not
+            // move loads across the asm statements)
+            const double* Ap = S + ((s * 4 + lc) * IR + lr) * PITCH;
+            double afq[FT_PF];
+#pragma unroll
+            for (int m = 0; m < FT_PF; ++m) afq[m] = Ap[m * 8 * PITCH];
 #pragma unroll
             for (int m = 0; m < FT_MT; ++m) {
-                const double af = S[((s * 4 + lc) * IR + m * 8 + lr) * PITCH];
+                const double af = afq[m % FT_PF];
+                if (m + FT_PF < FT_MT) afq[m % FT_PF] = Ap[(m + FT_PF) * 8 * PITCH];
 #pragma unroll
                 for (int n = 0; n < NK; ++n) dmma884k(acc[m][n][0], acc[m][n][1], af, bf[n]);
             }
@@ -495,9 +503,14 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
             double acc2[NK][2];
 #pragma unroll
             for (int n = 0; n < NK; ++n) { acc2[n][0] = 0.0; acc2[n][1] = 0.0; }
+            const double* Atp = S + (lr * IR + lc) * PITCH;
+            double atq[FT_PF];
+#pragma unroll
+            for (int q = 0; q < FT_PF; ++q) atq[q] = Atp[q * 4 * PITCH];
 #pragma unroll
             for (int q = 0; q < IR / 4; ++q) {
-                const double af = S[(lr * IR + q * 4 + lc) * PITCH];
+                const double af = atq[q % FT_PF];
+                if (q + FT_PF < IR / 4) atq[q % FT_PF] = Atp[(q + FT_PF) * 4 * PITCH];
 #pragma unroll
                 for (int n = 0; n < NK; ++n) dmma884k(acc2[n][0], acc2[n][1], af, breg[q][n]);
             }

@@ -104,26 +104,33 @@ cudaError_t launch_hxc_potential(const double* vh, const double* f0, const doubl
     return cudaGetLastError();
 }
 
+// One CTA = one chunk of 32 grid points, all functions: the chunk's nocc*kc rows of 256 bytes are one contiguous run of `out`.
 __global__ void out_init_kernel(const double* __restrict__ phi, const double* __restrict__ V, const double* __restrict__ vloc,
-                                const double* __restrict__ a, int nocc, int kc, long nr, long nrp, double* __restrict__ out) {
-    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;      // r runs over the padded chunks
-    if (r >= nrp) return;
-    const int f = blockIdx.y;
-    const int v = f / kc, kk = f - v * kc;
-    const long o = (r >> 5) * ((long)nocc * kc * CHUNK) + (long)f * CHUNK + (r & (CHUNK - 1));
-    double y = 0.0;
-    if (r < nr) {
-        if (V) y = phi[(long)v * nr + r] * V[(long)kk * nr + r];
-        if (vloc) y = fma(vloc[r], a[o], y);
+                                const double* __restrict__ a, int nocc, int kc, long nr, double* __restrict__ out) {
+    const long chunk = blockIdx.x;
+    const int lane = threadIdx.x & (CHUNK - 1), sub = threadIdx.x / CHUNK, nsub = blockDim.x / CHUNK;
+    const long r = chunk * CHUNK + lane;
+    const bool live = r < nr;
+    const long base = chunk * ((long)nocc * kc * CHUNK) + lane;
+    const double vl = (vloc && live) ? vloc[r] : 0.0;
+    for (int v = sub; v < nocc; v += nsub) {
+        const double p = (V && live) ? phi[(long)v * nr + r] : 0.0;
+        for (int kk = 0; kk < kc; ++kk) {
+            const long o = base + ((long)v * kc + kk) * CHUNK;
+            double y = 0.0;
+            if (live) {
+                if (V) y = p * __ldg(V + (long)kk * nr + r);
+                if (vloc) y = fma(vl, a[o], y);
+            }
+            out[o] = y;
+        }
     }
-    out[o] = y;
 }
 cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
                             double* out, cudaStream_t st) {
-    const long nrp = (nr + CHUNK - 1) / CHUNK * CHUNK;
-    if (!V && !vloc) return cudaMemsetAsync(out, 0, sizeof(double) * nrp * nocc * kc, st);
-    dim3 grid((unsigned)(nrp / 256 + (nrp % 256 ? 1 : 0)), (unsigned)(nocc * kc));
-    out_init_kernel<<<grid, 256, 0, st>>>(phi, V, vloc, a, nocc, kc, nr, nrp, out);
+    const long nchunks = (nr + CHUNK - 1) / CHUNK;
+    if (!V && !vloc) return cudaMemsetAsync(out, 0, sizeof(double) * nchunks * CHUNK * nocc * kc, st);
+    out_init_kernel<<<(unsigned)nchunks, 256, 0, st>>>(phi, V, vloc, a, nocc, kc, nr, out);
     return cudaGetLastError();
 }
 

@@ -423,6 +423,7 @@ int tddft_destroy(tddft_ctx* c) {
     for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
     cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
+    cudaFree(c->host_dx); cudaFree(c->host_dax);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (int i = 0; i < 2; ++i) { if (c->ev_x_ready[i]) cudaEventDestroy(c->ev_x_ready[i]); if (c->ev_ax_done[i]) cudaEventDestroy(c->ev_ax_done[i]); }
     for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); cudaFree(c->tiles[s].d_pslot); }
@@ -566,10 +567,15 @@ int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int 
     const long L = vector_len(c, mode);
     if (L < 0) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
     const size_t bytes = sizeof(cplx) * (size_t)L * nvec;
-    double *dX = nullptr, *dAX = nullptr;
-    if (cudaMalloc((void**)&dX, bytes) != cudaSuccess || cudaMalloc((void**)&dAX, bytes) != cudaSuccess) {
-        cudaGetLastError(); cudaFree(dX); return set_err(c, TDDFT_ENOMEM, "apply_host: device allocation failed");
+    if (c->host_bytes < bytes) {      // staging buffers are kept between calls (allocation and release of GBs costs milliseconds)
+        cudaFree(c->host_dx); cudaFree(c->host_dax); c->host_dx = c->host_dax = nullptr; c->host_bytes = 0;
+        if (cudaMalloc((void**)&c->host_dx, bytes) != cudaSuccess || cudaMalloc((void**)&c->host_dax, bytes) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(c->host_dx); c->host_dx = nullptr;
+            return set_err(c, TDDFT_ENOMEM, "apply_host: device allocation failed");
+        }
+        c->host_bytes = bytes;
     }
+    double *dX = c->host_dx, *dAX = c->host_dax;
     // The spin blocks of a spin-conserving vector are processed one after the other (apply_liouville_dev), so block 1 of X
     // is copied in while block 0 is computed and block 0 of AX is copied out while block 1 is computed: the copies run on
     // their own stream as 2-D copies (nvec rows of one block, pitch = one trial vector), ordered by events.
@@ -611,7 +617,6 @@ int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int 
     if (cudaStreamSynchronize(c->copy_stream) != cudaSuccess && !rc) rc = set_err(c, TDDFT_ECUDA, "apply_host: copy stream failed");
     if (cudaStreamSynchronize(c->stream) != cudaSuccess && !rc) rc = set_err(c, TDDFT_ECUDA, "apply_host: stream failed");
     if (start) cudaEventDestroy(start);
-    cudaFree(dX); cudaFree(dAX);
     return rc;
 }
 

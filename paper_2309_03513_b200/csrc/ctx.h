@@ -56,6 +56,7 @@ struct tddft_ctx {
     // host-buffer entry point: copies run on their own stream, block by block, behind the kernels (api.cu)
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_x_ready[2] = {nullptr, nullptr}, ev_ax_done[2] = {nullptr, nullptr};
+    double *host_dx = nullptr, *host_dax = nullptr; size_t host_bytes = 0;   // device staging of the host entry point (kept between calls)
     bool overlap_copies = false;     // set only while tddft_apply_liouville_host drives an apply
     // bookkeeping
     tddft_stats stats{};

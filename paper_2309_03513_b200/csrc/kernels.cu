@@ -436,7 +436,7 @@ contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, con
                 for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH) {
                     if (i < ti) {
                         const int lo = min(i, col), hi = max(i, col);
-                        cp_async16(dst, tau_c + ((long)lo * (2 * tj - lo + 1) / 2 + (hi - lo)) * CHUNK + lp2);
+                        cp_async16(dst, tau_c + (long)(lo * (2 * tj - lo + 1) / 2 + (hi - lo)) * CHUNK + lp2);     // slots fit 32 bits
                     } else *(double2*)dst = make_double2(0.0, 0.0);
                 }
             } else {

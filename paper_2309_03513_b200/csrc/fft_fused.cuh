@@ -124,6 +124,8 @@ __device__ __forceinline__ void bulk_g2s(void* smem, const void* gmem, unsigned 
 template <class L> struct HasColMap { static constexpr bool value = false; };      // loads that go through the pruned column map
 template <> struct HasColMap<LoadWorkC> { static constexpr bool value = true; };
 template <> struct HasColMap<LoadWorkT> { static constexpr bool value = true; };
+template <class S> struct StoresColMap { static constexpr bool value = false; };  // stores that go through the pruned column map
+template <> struct StoresColMap<StoreWorkC> { static constexpr bool value = true; };
 template <class L> struct IsStaged { static constexpr bool value = false; };
 template <> struct IsStaged<LoadWorkT> { static constexpr bool value = true; };
 struct BLoadPair {
@@ -272,6 +274,30 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
             for (int i = 0; i < R2y; ++i) ccol[r][i] = (t < NZ * R1y) ? __ldg(ld.cmap + (k1 * R2y + i) * NZ + zp) : -1;
         }
     }
+    // forward kernels storing to pruned work grids: the thread's 16-bit column indices of the last stage, two per register
+    constexpr bool SCOLS = StoresColMap<Store>::value && !INV;
+    static_assert(!SCOLS || NY * NZ < 65535, "16-bit column indices");
+    unsigned scol[SCOLS ? NR0 : 1][(R2y + 1) / 2];
+    if constexpr (SCOLS) {
+#pragma unroll
+        for (int r = 0; r < NR0; ++r) {
+            const int t = tid + r * NTHR;
+            const int k1 = t / NZ, zp = t - k1 * NZ;
+#pragma unroll
+            for (int h = 0; h < (R2y + 1) / 2; ++h) {
+                unsigned pk = 0xffffffffu;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int k = 2 * h + e;
+                    int cc = -1;
+                    if (k < R2y && t < NZ * R1y) cc = __ldg(st.cmap + (k1 * R2y + k) * NZ + zp);
+                    const unsigned v = cc < 0 ? 0xffffu : (unsigned)cc;
+                    pk = e == 0 ? ((pk & 0xffff0000u) | v) : ((pk & 0x0000ffffu) | (v << 16));
+                }
+                scol[r][h] = pk;
+            }
+        }
+    }
     static_assert(!STAGED || INV, "only the inverse kernel reads staged work grids");
     cplx* stage = sm + NY * PITCH;                      // STAGED: [ncols] compact plane, then the mbarrier
     unsigned long long* mbar = nullptr;
@@ -356,6 +382,25 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                 });
             __syncthreads();
             // y stage 2 (radix R2y): shared -> registers -> global, lanes run over z (coalesced rows)
+            if constexpr (SCOLS) {
+#pragma unroll
+                for (int r = 0; r < NR0; ++r) {
+                    const int t = tid + r * NTHR;
+                    if (t < NZ * R1y) {
+                        const int k1 = t / NZ, zp = t - k1 * NZ;
+                        const cplx* col = sm + TZ::pad(zp) + (k1 * R2y) * PITCH;
+                        cplx x[R2y];
+#pragma unroll
+                        for (int i = 0; i < R2y; ++i) x[i] = col[i * PITCH];
+                        Dft<R2y, false>::run(x);
+#pragma unroll
+                        for (int k = 0; k < R2y; ++k) {
+                            const unsigned cc = (scol[r][k / 2] >> (16 * (k & 1))) & 0xffffu;
+                            if (cc != 0xffffu) st_pol(S.g + cc, x[k], S.pol);
+                        }
+                    }
+                }
+            } else
             run_rounds<NZ * R1y, NTHR, DB2, RegBuf<cplx, R2y>>(tid,
                 [&](int t, RegBuf<cplx, R2y>& q) {
                     const int k1 = t / NZ, zp = t - k1 * NZ;

@@ -358,14 +358,14 @@ cudaError_t launch_contract_dual(double* out, const double* a, const double* tau
 
 // ------------------------------------------------------------------------------------------------------
 // S5, register-resident tiles.  One warp owns ONE grid point and keeps the whole row block of the tile in registers:
-// the accumulators of out[I] (up to 112 rows x 16 trial vectors = 56 registers per lane) and, for off-diagonal tiles,
-// the B fragments of a[I] (54 registers) that the transposed product out[J] += tau^T a[I] needs.  The CTA (8 warps =
-// 8 points) sweeps the columns of the tile 8 at a time through a double-buffered cp.async stage (tau[all i][8 j] and
-// a[8 j][16 k], 64-byte rows padded to 80 bytes); every tau element is loaded into the SM once and used for both
-// directions: 110 DMMAs per warp between barriers and ~0.14 bytes of L2->SM traffic per flop instead of 0.375.
-// Row pitch 10 doubles and 108 rows per column make (row stride) = 8 mod 16 doubles, so both fragment patterns
-// (lanes over (i, j) for tau and over (j, i) for tau^T) spread over 8 distinct 8-byte banks: 4 wavefronts per load.
-// Results leave through shared memory so that every global access is a full 64-byte row.
+// the accumulators of out[I] (up to 112 rows x 16 trial vectors = 56 doubles per lane) and, for off-diagonal tiles,
+// the B fragments of a[I] (54 doubles) that the transposed product out[J] += tau^T a[I] needs.  The CTA (FT_P = 4 warps =
+// 4 consecutive points, two CTAs per SM) sweeps the columns of the tile 8 at a time through a double-buffered cp.async
+// stage (tau[all i][8 j] and a[8 j][16 k], 32-byte rows padded to 48 bytes); every tau element is loaded into the SM once
+// and used for both directions: 110 DMMAs per warp between barriers and ~0.14 bytes of L2->SM traffic per flop instead
+// of 0.375.  Row pitch FT_PITCH = 6 doubles and 108 rows per column make (row stride) = 8 mod 16 doubles, so both
+// fragment patterns (lanes over (i, j) for tau and over (j, i) for tau^T) spread over 8 distinct 8-byte banks: 4
+// wavefronts per load.  Results leave through shared memory so that every global access is a full 32-byte row.
 // Tile shapes: MT row tiles of 8 per warp, IR rows per column in a stage (= largest row block; IR = 4 mod 8 for the bank pattern).
 // The smaller shape leaves registers for the compiler to run fragment loads ahead of the DMMAs.
 struct FullShapeL { static constexpr int MT = 14, IR = 108; };

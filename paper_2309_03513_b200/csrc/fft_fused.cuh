@@ -244,8 +244,9 @@ template <int NTHR, int MINB> struct PlaneRegs {
 };
 
 // ---- plane kernel -------------------------------------------------------------------------------------------
-// Persistent CTAs walk over the units (packed grid b, plane x), unit u = b*NX + x.  Flat index of (x, y, z) inside
-// a grid: (x*NY + y)*NZ + z.
+// Persistent CTAs walk over the units (packed grid b, plane x) plane-major, unit u = x*batch + b: the CTAs running at the same
+// time then work on the same few planes of all grids of the launch, and the orbital planes the pairs of a sub-block share
+// are read from DRAM once and found in L2 (or L1) by the other pairs.  Flat index of (x, y, z) inside a grid: (x*NY + y)*NZ + z.
 template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
 __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::value)) plane_kernel(Load ld, Store st, int nx, int nunits, int l2pf, const cplx* __restrict__ twy_g, const cplx* __restrict__ twz_g) {
     using TY = Two<NY>; using TZ = Two<NZ>;
@@ -263,6 +264,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
     typedef decltype(bind(ld, 0, 0, 0L)) BL;
     typedef typename BL::Raw Raw;
     constexpr bool STAGED = IsStaged<Load>::value;
+    const int nbatch = nunits / nx;
     constexpr int NR0 = (NZ * R1y + NTHR - 1) / NTHR;   // rounds of the first inverse stage
     int ccol[HasColMap<Load>::value ? NR0 : 1][R2y];
     if constexpr (HasColMap<Load>::value) {
@@ -307,7 +309,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
         if (tid == 0) {
             mbar_init(mbar, 1);
             if ((int)blockIdx.x < nunits) {
-                const int b0 = blockIdx.x / nx, x0 = blockIdx.x - b0 * nx;
+                const int x0 = blockIdx.x / nbatch, b0 = blockIdx.x - x0 * nbatch;
                 mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
                 bulk_g2s(stage, ld.work + (long)b0 * ld.gstride + (long)x0 * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
             }
@@ -316,13 +318,13 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
     }
 
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
-        const int b = u / nx, xpl = u - b * nx;
+        const int xpl = u / nbatch, b = u - xpl * nbatch;
         BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
         if constexpr (STAGED) { L.stage = stage; mbar_wait(mbar, parity); parity ^= 1; }
         const auto S = bind(st, b, xpl, (long)xpl * NY * NZ);
         {   // operands of the unit this CTA takes next -> L2
             const int un = u + gridDim.x;
-            if (l2pf && un < nunits) { const int bn = un / nx, xn = un - bn * nx; bind(ld, bn, xn, (long)xn * NY * NZ).prefetch_l2(NY * NZ, tid, NTHR); }
+            if (l2pf && un < nunits) { const int xn = un / nbatch, bn = un - xn * nbatch; bind(ld, bn, xn, (long)xn * NY * NZ).prefetch_l2(NY * NZ, tid, NTHR); }
         }
         if constexpr (!INV) {
             // z stage 1 (radix R1z, twiddle after): global -> registers -> shared
@@ -452,7 +454,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
             if constexpr (STAGED) {     // the stage is consumed: start the copy of this CTA's next unit behind the remaining stages
                 const int un = u + gridDim.x;
                 if (tid == 0 && un < nunits) {
-                    const int bn = un / nx, xn = un - bn * nx;
+                    const int xn = un / nbatch, bn = un - xn * nbatch;
                     mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
                     bulk_g2s(stage, ld.work + (long)bn * ld.gstride + (long)xn * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
                 }

@@ -473,12 +473,13 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         { const char* e = getenv("TDDFT_CT_FULL"); c->ct_full = !(e && atoi(e) == 0); }
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) {
-            // latency-bound kernels: large launches beat L2 residency (measured); among the sizes up to 64 grids and 384 MB
-            // take the one whose plane units (n1 per grid) fill whole waves of two CTAs per SM
-            const long cap = std::max<long>(1, std::min<long>(64, (384L << 20) / (16 * nr)));
+            // large launches win (measured up to 192 grids): with the plane-major unit order the CTAs of a launch share orbital
+            // planes whatever its size, and launch tails shrink; up to 96 grids and 640 MB of work grids, among the upper
+            // quarter the size whose plane units (n1 per grid) fill whole waves of two CTAs per SM best
+            const long cap = std::max<long>(1, std::min<long>(96, (640L << 20) / (16 * nr)));
             const long resident = 2L * c->num_sms;
             long bestb = cap; double beste = 0.0;
-            for (long b = cap; b >= std::max<long>(1, cap / 2); --b) {
+            for (long b = cap; b >= std::max<long>(1, cap - cap / 4); --b) {
                 int si, sj; choose_subblock((int)(2 * b), &si, &sj);
                 const long units = (long)(si * sj + 1) / 2 * grid[0], waves = (units + resident - 1) / resident;   // grids a pair launch really holds
                 const double e = (double)units / (double)(waves * resident);

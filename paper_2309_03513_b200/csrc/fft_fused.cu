@@ -12,9 +12,9 @@ namespace tddft {
 #define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2, 648) X(48, 48, 96, 5, 0) X(24, 24, 96, 8, 0) X(18, 20, 96, 8, 0)
 #define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
 
-static int plane_variant() {          // tuning switch TDDFT_VAR: bit 0 persistent grid, bit 3 L2 prefetch of the next unit's orbital planes, bit 4 of its work-grid plane, bit 5 evict-first L2 policy on the work-grid / tau / a(r) streams, bit 6 TMA-staged inverse plane kernel
+static int plane_variant() {          // tuning switch TDDFT_VAR: bit 0 persistent grid, bit 3 L2 prefetch of the next unit's orbital planes (off: they are shared with the units running now), bit 4 of its work-grid plane, bit 5 evict-first L2 policy on the work-grid / tau / a(r) streams, bit 6 TMA-staged inverse plane kernel
     static int v = -1;
-    if (v < 0) { const char* e = getenv("TDDFT_VAR"); v = e ? atoi(e) : 57; }
+    if (v < 0) { const char* e = getenv("TDDFT_VAR"); v = e ? atoi(e) : 49; }
     return v;
 }
 template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
@@ -62,7 +62,7 @@ static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArg
         return cudaErrorInvalidValue;
     }
     if constexpr (TSTAGED > 0) {
-        // staged variant (TDDFT_VAR bit 6, default on) when the plane, the stage and the barrier fit one CTA's shared memory
+        // staged variant (TDDFT_VAR bit 6, opt-in) when the plane, the stage and the barrier fit one CTA's shared memory
         const size_t need = sizeof(cplx) * ((size_t)NY * Two<NZ>::PITCH + (size_t)a.ncols) + 16;
         if (skind == ZS_SPLIT2 && (plane_variant() & 64) && need <= 227 * 1024)
             return plane_launch<NY, NZ, TSTAGED, 1, true>(LoadWorkT{a.work, a.wstride, a.cmap, a.ncols, hint}, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);

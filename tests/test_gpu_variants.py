@@ -24,7 +24,7 @@ print("variant ok")
 """
 
 
-@pytest.mark.parametrize("env", [{"TDDFT_VAR": "121"}, {"TDDFT_CT_FULL": "0"}, {"TDDFT_VAR": "0"}])
+@pytest.mark.parametrize("env", [{"TDDFT_VAR": "113"}, {"TDDFT_CT_FULL": "0"}, {"TDDFT_VAR": "0"}])
 def test_variant_parity_on_the_bench_grid(env):
     e = dict(os.environ); e.update(env)
     r = subprocess.run([sys.executable, "-c", SCRIPT % {"root": ROOT}], env=e, capture_output=True, text=True, timeout=600)

@@ -22,9 +22,9 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the three S4 kernels per batch of 80 pairs at NV215, from the ncu --set full
-# capture summarised in profiles/r01g_summary.md (179.5 + 245.4 + 335.5 MB), per pair
-NCU_TRAFFIC_PER_PAIR = 760.4e6 / 80
+# dram__bytes_read.sum + dram__bytes_write.sum of the three S4 kernels per batch of 180 pairs at NV215, from the ncu --set full
+# capture summarised in profiles/r01i_summary.md (361.2 + 623.9 + 822.7 MB), per pair
+NCU_TRAFFIC_PER_PAIR = 1807.8e6 / 180
 METRIC = "liouville_vector_applies_per_s"
 UNIT = "vector-applies/s"
 

@@ -101,7 +101,7 @@ def oracle_sample(cfg, sample_nocc=6):
     the time is scaled by (sum_s nocc_s^2) / (sum_s sample_nocc^2)."""
     from oracle import lattice as olat
     from oracle import liouville as olv
-    from paper_2309_03513_b200 import inputs
+    import synthetic_inputs as inputs
     miller, g2 = olat.enumerate_half_sphere(cfg["lattice"], cfg["ecut"])
     rng = np.random.Generator(np.random.PCG64(cfg["seed"]))
     nsp = cfg["nspin"]
@@ -172,7 +172,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=0)
     args = ap.parse_args()
 
-    from paper_2309_03513_b200 import inputs
+    import synthetic_inputs as inputs
     cfg = inputs.config(args.config)
     if args.nocc:
         cfg["nocc"] = tuple(args.nocc)

@@ -22,10 +22,24 @@ Spin flip, up-occupied -> down-virtual (Eqs. 21, 23, 25; readi
 vector {x_v : v = 1..N_up}; y(r) = -alpha sum_v' a_v'(r) C[phi_v,up phi_v',up](r);
 y(G) += (|G|^2/2 - eps_v,up) x_v(G) [+ V_loc,dn a_v]; projected with Phi_dn.  No Hartree, no f_xc (north star).
 
+Options beyond the TDA north-star path (each default reproduces the path above exactly):
+  sf_xc_kernel  spin flip keeps K1e^SF (Eq. 24) with the kernel of Eq. 26,
+                f^SF(r) = (V_xc,s(r) - V_xc,s~(r)) / (rho_s(r) - rho_s~(r)), set to zero where |rho_up - rho_dn| < sf_cut
+                ("1e-3", no unit given; reading A9 takes e/bohr^3):
+                y(r) += phi_v,s~(r) f^SF(r) sum_v' phi_v',s~(r) a_v'(r)
+  pair_mask     near-sightedness truncation: the pair potentials tau_mn with mask[m, n] False are
+                taken as zero in K1d
+  wannier_u     Eq. 31: phi_v = sum_n U_vn phi~_n; K1d is evaluated with the rotated orbitals,
+                (K1d A)_v = alpha P_c sum_m U_vm { sum_n a~_n tau~_mn },  a~_n = sum_v' U_v'n a_v' (real U), and the
+                mask then refers to pairs (m, n) of ROTATED orbitals, as in the paper
+  ace           D uses H = T + V_loc + alpha V_X^ACE (Eqs. 28-30; oracle/ace.py)
+`coupling` is the off-diagonal block K2e - K2d of Eq. 1 (Eqs. 5, 7; at Gamma with real functions
+K2e = K1e; spin flip: Eqs. S7, S9, which read the trial vector of the OPPOSITE flip direction).
+
 Vector layout (same as the C ABI): one trial vector = [spin][v][g] complex, contiguous;
 a block is [k][spin][v][g].
 
-Pins: tests/test_oracle_liouville.py.  Parity against numbers printed by the paper: unpinned
+Pins: tests/test_oracle_liouville.py, tests/test_oracle_extensions.py.  Parity against numbers printed by the paper: unpinned
 (the paper prints none for this operator); pinned instead by closed forms (plane-wave pair potential,
 Hartree of a cosine, D on plane-wave orbitals), brute-force O(N_r^2) evaluation, Eq. 31 invariance,
 symmetry of A, linearity in alpha, nspin=1 vs duplicated nspin=2.
@@ -43,7 +57,8 @@ SPIN_FLIP_DOWN_UP = 2   # down occupied -> up virtual
 
 class Problem:
     def __init__(self, lattice, grid, ecut_ry, nspin, psi, eig, alpha,
-                 use_hartree_fxc=True, rho_floor=1e-10, vloc=None, fft_backend="radix"):
+                 use_hartree_fxc=True, rho_floor=1e-10, vloc=None, fft_backend="radix",
+                 sf_xc_kernel=False, sf_cut=1e-3, pair_mask=None, wannier_u=None, ace=None):
         self.A = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
         self.grid = tuple(int(n) for n in grid)
         self.nr = self.grid[0] * self.grid[1] * self.grid[2]
@@ -83,6 +98,20 @@ class Problem:
         else:
             self.rho0 = rho
         self.fuu, self.fud, self.fdd = lda.fxc(self.rho0[0], self.rho0[1], rho_floor)
+        # options of SURVEY 8(f)
+        self.sf_xc_kernel = bool(sf_xc_kernel)
+        self.fsf = None
+        if self.sf_xc_kernel:                                                       # Eq. 26
+            vu, vd = lda.vxc(np.maximum(self.rho0[0], rho_floor), np.maximum(self.rho0[1], rho_floor))
+            d = self.rho0[0] - self.rho0[1]
+            ok = np.abs(d) >= sf_cut
+            self.fsf = np.where(ok, (vu - vd) / np.where(ok, d, 1.0), 0.0)
+        self.pair_mask = None if pair_mask is None else [np.asarray(m, dtype=bool) for m in pair_mask]
+        self.U = None if wannier_u is None else [np.asarray(u, dtype=np.float64) for u in wannier_u]
+        self.phi_rot = None
+        if self.U is not None:                                                      # phi~_n = sum_v U_vn phi_v
+            self.phi_rot = [np.tensordot(self.U[s].T, self.phi[s], axes=1) for s in range(self.nspin)]
+        self.ace = ace          # list over spins of xi [n_ace, npwh] (oracle/ace.py) or None
 
     # ---- representation changes -------------------------------------------------
     def to_real(self, c):
@@ -136,7 +165,24 @@ class Problem:
         """O3-O5 for one trial vector: everything a column of A x needs that is shared by all columns."""
         xs = self.split(x, mode)
         a = [np.stack([self.to_real(c) for c in blk]) for blk in xs]          # O3
-        ctx = dict(mode=mode, x=xs, a=a, V=None)
+        ctx = dict(mode=mode, x=xs, a=a, V=None, k1d_rot=None, Vsf=None)
+        if self.U is not None and self.alpha != 0.0:
+            # Eq. 31: g_m(r) = sum_n a~_n(r) tau~_mn(r) for every rotated orbital m of each block (N^2 pair potentials)
+            ctx["k1d_rot"] = []
+            for b in range(len(xs)):
+                s_occ = b if mode == SPIN_CONSERVING else (0 if mode == SPIN_FLIP else 1)
+                U, pr = self.U[s_occ], self.phi_rot[s_occ]
+                at = np.tensordot(U.T, a[b], axes=1)                                  # a~_n = sum_v' U_v'n a_v'
+                g = np.zeros_like(at)
+                for m in range(self.nocc[s_occ]):
+                    for n in range(self.nocc[s_occ]):
+                        if self.pair_mask is not None and not self.pair_mask[s_occ][m, n]:
+                            continue
+                        g[m] += at[n] * self.coulomb(pr[m] * pr[n])
+                ctx["k1d_rot"].append(g)
+        if mode != SPIN_CONSERVING and self.sf_xc_kernel:                            # Eq. 22 and Eq. 24
+            s_occ = 0 if mode == SPIN_FLIP else 1
+            ctx["Vsf"] = self.fsf * np.sum(self.phi[s_occ] * a[0], axis=0)
         if mode == SPIN_CONSERVING and self.use_hartree_fxc:
             drho = [np.sum(self.phi[s] * a[s], axis=0) for s in range(self.nspin)]   # O4
             if self.nspin == 2:
@@ -165,13 +211,24 @@ class Problem:
         y = np.zeros(self.grid)
         if ctx["V"] is not None:
             y += phi[v] * ctx["V"][s]
-        for vp in range(self.nocc[s_occ]):                                            # O6
-            tau = self.coulomb(phi[v] * phi[vp])
-            y -= self.alpha * a[vp] * tau
+        if ctx["Vsf"] is not None:
+            y += phi[v] * ctx["Vsf"]
+        if ctx["k1d_rot"] is not None:                                                # Eq. 31, outer sum over m
+            y -= self.alpha * np.tensordot(self.U[s_occ][v], ctx["k1d_rot"][blk], axes=1)
+        elif self.alpha != 0.0:
+            for vp in range(self.nocc[s_occ]):                                        # O6
+                if self.pair_mask is not None and not self.pair_mask[s_occ][v, vp]:
+                    continue
+                tau = self.coulomb(phi[v] * phi[vp])
+                y -= self.alpha * a[vp] * tau
         if self.vloc is not None:
             y += self.vloc[s_tgt] * a[v]
         yg = self.to_sphere(y)                                                        # O7
         yg = yg + (0.5 * self.g2 - self.eig[s_occ][v]) * ctx["x"][blk][v]             # O8
+        if self.ace is not None:                                                      # alpha V_X^ACE a_v, Eq. 29
+            xv = ctx["x"][blk][v]
+            for xi in self.ace[s_tgt]:
+                yg = yg - self.alpha * xi * (2.0 * np.real(np.vdot(xi, xv)) - xi[0].real * xv[0].real)
         return self.project_c(yg, s_tgt)                                              # O9
 
     def apply(self, X, mode=SPIN_CONSERVING):
@@ -186,6 +243,51 @@ class Problem:
             for s in range(len(ctx["x"])):
                 for v in range(ctx["x"][s].shape[0]):
                     out[k, o:o + self.npwh] = self.column(ctx, s, v)
+                    o += self.npwh
+        return out
+
+    # ---- off-diagonal block of Eq. 1 ------------------------------------------------
+    def coupling(self, X, mode=SPIN_CONSERVING):
+        """(K2e - K2d) X, block of trial vectors (Eqs. 5, 7; spin flip Eqs. S7, S9).
+
+        Spin conserving: (K2e X)_v = P_c phi_v V[X] with the same V as K1e (real functions: a* phi = phi* a);
+        (K2d X)_v = alpha P_c sum_v' phi_v'(r) C[a_v' phi_v](r).
+        Spin flip, output in the layout of `mode` (functions v over the occupied orbitals of s~, living in s): the input X
+        is a block of trial vectors of the OPPOSITE flip direction (functions v' over the occupied orbitals of s, living in
+        s~):  (K2d X)_v = alpha P_c,s sum_{v' in occ s} phi_v's(r) C[a_v' phi_v,s~](r), and with sf_xc_kernel
+        (K2e X)_v = P_c,s phi_v,s~ f^SF sum_{v' in occ s} a_v' phi_v's."""
+        X = np.asarray(X, dtype=np.complex128)
+        in_mode = mode if mode == SPIN_CONSERVING else (SPIN_FLIP_DOWN_UP if mode == SPIN_FLIP else SPIN_FLIP)
+        X = X.reshape(-1, self.vector_len(in_mode))
+        out = np.zeros((X.shape[0], self.vector_len(mode)), dtype=np.complex128)
+        for k in range(X.shape[0]):
+            xs = self.split(X[k], in_mode)
+            a = [np.stack([self.to_real(c) for c in blk]) for blk in xs]
+            o = 0
+            if mode == SPIN_CONSERVING:
+                V = self.prepare(X[k], mode)["V"]
+                for s in range(self.nspin):
+                    for v in range(self.nocc[s]):
+                        y = np.zeros(self.grid)
+                        if V is not None:
+                            y += self.phi[s][v] * V[s]
+                        for vp in range(self.nocc[s]):
+                            y -= self.alpha * self.phi[s][vp] * self.coulomb(a[s][vp] * self.phi[s][v])
+                        out[k, o:o + self.npwh] = self.project_c(self.to_sphere(y), s)
+                        o += self.npwh
+            else:
+                s_occ = 0 if mode == SPIN_FLIP else 1       # s~ of the OUTPUT: its functions run over occ(s~), live in s
+                s_tgt = 1 - s_occ
+                Vsf = None
+                if self.sf_xc_kernel:
+                    Vsf = self.fsf * np.sum(self.phi[s_tgt] * a[0], axis=0)
+                for v in range(self.nocc[s_occ]):
+                    y = np.zeros(self.grid)
+                    if Vsf is not None:
+                        y += self.phi[s_occ][v] * Vsf
+                    for vp in range(self.nocc[s_tgt]):
+                        y -= self.alpha * self.phi[s_tgt][vp] * self.coulomb(a[0][vp] * self.phi[s_occ][v])
+                    out[k, o:o + self.npwh] = self.project_c(self.to_sphere(y), s_tgt)
                     o += self.npwh
         return out
 

@@ -3,7 +3,7 @@ import numpy as np
 
 from oracle import lattice as olat
 from oracle import liouville as olv
-from paper_2309_03513_b200 import inputs
+import synthetic_inputs as inputs
 
 
 class Case:

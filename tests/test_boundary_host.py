@@ -110,7 +110,7 @@ def test_bench_sharding_two_ranks_gloo(tmp_path):
 import os, sys
 sys.path.insert(0, %r)
 import numpy as np, torch, torch.distributed as dist
-from paper_2309_03513_b200 import inputs
+import synthetic_inputs as inputs
 from oracle import lattice as olat
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()

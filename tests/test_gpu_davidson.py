@@ -41,7 +41,7 @@ def test_davidson_config1_restart_and_own_start():
     # force restarts; CUDA with the library's own start vectors.  All must give the same eigenvalues.
     import torch
     from paper_2309_03513_b200 import binding as b
-    from paper_2309_03513_b200 import inputs
+    import synthetic_inputs as inputs
     nroots = 3
     base = Case.from_config(1)
     x0 = inputs.diagonal_guess(base.rng, base.oracle.precond_diag(0), base.npwh, 2 * nroots)

@@ -5,7 +5,7 @@ import pytest
 from oracle import lattice as lat
 from oracle import liouville as lv
 from oracle.davidson import davidson
-from paper_2309_03513_b200 import inputs
+import synthetic_inputs as inputs
 
 
 def test_d_only_closed_form():

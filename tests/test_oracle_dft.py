@@ -56,8 +56,10 @@ def test_round_trip_and_parseval():
 
 def test_backends_agree_on_config_grids():
     rng = np.random.default_rng(3)
-    for shape in [(24, 24, 24), (48, 48, 48)]:
-        x = rng.standard_normal(shape)
-        a = fft3(x, -1)
-        b = fft3(x, -1, backend="numpy")
-        assert np.max(np.abs(a - b)) < 1e-12 * np.max(np.abs(b))
+    # every grid the sampled-column parity checks use the library backend on, both signs, complex input
+    for shape in [(24, 24, 24), (48, 48, 48), (72, 72, 72), (96, 96, 100)]:
+        x = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+        for sign in (-1, +1):
+            a = fft3(x, sign)
+            b = fft3(x, sign, backend="numpy")
+            assert np.max(np.abs(a - b)) < 1e-12 * np.max(np.abs(b))

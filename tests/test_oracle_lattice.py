@@ -88,3 +88,18 @@ def test_grid_g2_matches_direct():
     g = 2 * B[0] - 2 * B[1] + 1 * B[2]      # index (2, 3, 1) -> m = (2, -2, 1)
     assert g2[2, 3, 1] == pytest.approx(np.dot(g, g), rel=1e-14)
     assert g2[0, 0, 0] == 0.0
+
+
+def test_grid_must_hold_the_sphere():
+    """check_grid_holds_sphere: 2 m_max + 1 <= n on every axis, and a grid one point short is refused by Problem."""
+    from oracle import liouville as olv
+    cubic = [[10.0, 0, 0], [0, 10.0, 0], [0, 0, 10.0]]
+    miller, g2 = lat.enumerate_half_sphere(cubic, 10.0)
+    mmax = np.abs(miller).max(0)
+    assert list(mmax) == [5, 5, 5]            # floor(sqrt(10) * 10 / (2 pi)) = 5
+    assert lat.check_grid_holds_sphere(miller, (11, 11, 11))
+    for short in [(10, 11, 11), (11, 10, 11), (11, 11, 10)]:
+        assert not lat.check_grid_holds_sphere(miller, short)
+    psi = [np.zeros((1, len(miller)), dtype=complex)]; psi[0][0, 0] = 1.0
+    with pytest.raises(ValueError):
+        olv.Problem(cubic, (12, 12, 10), 10.0, 1, psi, [np.array([-0.1])], 0.0)

@@ -68,3 +68,27 @@ def test_spin_exchange_symmetry_and_floor():
     assert np.allclose(a[0], b[2]) and np.allclose(a[1], b[1]) and np.allclose(a[2], b[0])
     f = lda.fxc(np.array([1e-12, 0.1]), np.array([0.1, 0.1]), rho_floor=1e-10)
     assert f[0][0] == 0 and f[1][0] == 0 and f[2][0] == 0 and f[0][1] != 0
+
+
+def test_spin_interpolation_normalisation():
+    """f(zeta) of reading A5 is normalised so that f(0) = 0 and f(1) = 1: the fully polarised gas has exactly the
+    PZ81 'P' correlation energy, the unpolarised one exactly 'U' (PAPER.md:770, :915 cite PZ81).  A wrong denominator
+    (2^(1/3) - 1, 2^(4/3) - 1, ...) passes the continuity / ordering checks above but fails here."""
+    for rs in (0.3, 1.0, 2.0, 7.5):
+        hd = lda.HyperDual(np.float64(rs))
+        eu, ep = float(lda._eps_c_pz(hd, lda.PZ_U).f), float(lda._eps_c_pz(hd, lda.PZ_P).f)
+        assert lda.eps_c(rs, 0.0) == eu
+        assert lda.eps_c(rs, 1.0) == pytest.approx(ep, rel=1e-15)
+        assert lda.eps_c(rs, -1.0) == pytest.approx(ep, rel=1e-15)
+        # the same through exc_density itself (the function fxc differentiates): e_xc - e_x = rho eps_c
+        rho = 3.0 / (4.0 * np.pi * rs ** 3)
+        ex_pol = -0.75 * (6.0 / np.pi) ** (1.0 / 3.0) * rho ** (4.0 / 3.0)
+        assert float(lda.exc_density(rho, 0.0).f) - ex_pol == pytest.approx(rho * ep, rel=1e-12)
+        ex_unp = -0.75 * (6.0 / np.pi) ** (1.0 / 3.0) * 2.0 * (rho / 2.0) ** (4.0 / 3.0)
+        assert float(lda.exc_density(rho / 2.0, rho / 2.0).f) - ex_unp == pytest.approx(rho * eu, rel=1e-12)
+    # value typed from the PZ81 formula: f(1/2) = [(3/2)^(4/3) + (1/2)^(4/3) - 2] / (2^(4/3) - 2) = 0.11394 / 0.51984 = 0.2191
+    hd = lda.HyperDual(np.float64(2.0))
+    eu, ep = float(lda._eps_c_pz(hd, lda.PZ_U).f), float(lda._eps_c_pz(hd, lda.PZ_P).f)
+    f_half = (1.5 ** (4.0 / 3.0) + 0.5 ** (4.0 / 3.0) - 2.0) / (2.0 ** (4.0 / 3.0) - 2.0)
+    assert f_half == pytest.approx(0.2191, abs=1e-4)
+    assert lda.eps_c(2.0, 0.5) == pytest.approx(eu + f_half * (ep - eu), rel=1e-14)

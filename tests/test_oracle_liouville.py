@@ -7,7 +7,7 @@ import pytest
 from oracle import lattice as lat
 from oracle import liouville as lv
 from oracle import lda
-from paper_2309_03513_b200 import inputs
+import synthetic_inputs as inputs
 
 HEX = [[9.0, 0, 0], [-4.5, 9.0 * math.sqrt(3) / 2, 0], [0, 0, 7.0]]
 TRI = [[4.0, 0, 0], [0.5, 4.2, 0], [0.3, -0.2, 4.5]]

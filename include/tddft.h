@@ -55,7 +55,8 @@ typedef enum {
   TDDFT_EUNSUPPORTED = 5   /* valid request this build cannot serve (e.g. an FFT length without a plan) */
 } tddft_status;
 
-/* All fields optional: pass NULL for defaults, or zero-initialise and set struct_size = sizeof(tddft_options). */
+/* All fields optional: pass NULL for defaults, or zero-initialise and set struct_size = sizeof(tddft_options).
+ * Pointers are read during tddft_init only, except vloc_* and x0 (borrowed for the life of the context). */
 typedef struct {
   int struct_size;          /* ABI versioning: sizeof(tddft_options) of the caller */
   int use_hartree_fxc;      /* spin-conserving K1e (Eq. 4): 1 = on (default), 0 = off; set -1 for "default" */
@@ -74,6 +75,29 @@ typedef struct {
   int n_x0;
   unsigned long long seed;  /* seed of the library's own start vectors */
   int fft_path;             /* 0 = fused plane/x kernels when the grid shape has them (default), 1 = general pass kernels only */
+  int block;                /* Davidson: most correction vectors appended per iteration; <= 0: nroots */
+  int precond;              /* Davidson preconditioner: 0 = projector-aware (reading A11b, default), 1 = diagonal */
+  int verbose;              /* 1: tddft_davidson prints one line per iteration on stderr */
+  /* Spin-flip xc kernel (Eqs. 24, 26; reading A9): 0 = off (default, north star), 1 = on */
+  int sf_xc_kernel;
+  double sf_cut;            /* f^SF = 0 where |rho_up - rho_dn| < sf_cut (e/bohr^3); <= 0: 1e-3 */
+  /* Near-sightedness truncation of K1d (Eqs. 31-32).
+   * wannier_u_*: HOST, [nocc][nocc] row-major real orthogonal U with phi_v = sum_n U[v][n] phi~_n; NULL = identity
+   *   (the orbitals handed to tddft_init are used as they are).  The real-space part of the operator then runs on the
+   *   rotated orbitals phi~ and rotated trial functions a~_n = sum_v U[v][n] a_v, and the result is rotated back.
+   * s_thr > 0: pairs (m, n) of (rotated) orbitals with overlap S_mn < s_thr (Eq. 32) are dropped (tau~_mn = 0).
+   * pair_list_*: HOST int[2*n_pairs_*], explicit unordered pairs (m, n) to keep; overrides s_thr for that spin;
+   *   NULL = all pairs m <= n.  A diagonal pair (m, m) is kept only if listed. */
+  const double* wannier_u_up; const double* wannier_u_dn;
+  double s_thr;
+  const int* pair_list_up; long n_pairs_up;
+  const int* pair_list_dn; long n_pairs_dn;
+  /* ACE exact exchange inside D (Eqs. 28-30): ace = 1 builds V_X^ACE per spin from the
+   * occupied orbitals plus n_ace_extra_* further orbitals (DEVICE complex128 [n_extra][npwh], orthonormal to the
+   * occupied ones, read during tddft_init only) and D uses H = T + V_loc + alpha V_X^ACE. */
+  int ace;
+  const double* psi_ace_up; int n_ace_extra_up;
+  const double* psi_ace_dn; int n_ace_extra_dn;
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,
@@ -121,16 +145,27 @@ int tddft_apply_liouville_host(tddft_ctx* ctx, const double* X_host, double* AX_
 int tddft_davidson(tddft_ctx* ctx, int nroots, int mode, double* evals, double* evecs, int* iters,
                    double* resnorms);
 
+/* Off-diagonal block of the full Casida matrix, BX = (K2e - K2d) X (Eq. 1; Eqs. 5, 7 PAPER.md:87-96;
+ * SURVEY 8(f)2).  At Gamma with real functions K2e = K1e; K2d is the (phi, a, phi) operand pattern:
+ * (K2d X)_v = alpha P_c sum_v' phi_v'(r) C[a_v' phi_v](r), N_occ^2 * nvec pair FFTs.
+ * mode = TDDFT_SPIN_CONSERVING: X and BX in the spin-conserving layout.  Spin flip (Eqs. S7, S9): BX is in
+ * the layout of `mode`, X is a block of trial vectors of the OPPOSITE flip direction.  X, BX: DEVICE, BX must not alias X.
+ * With A X from tddft_apply_liouville the full operator of Eq. 1 is (A X + B Y, B X + A Y). */
+int tddft_apply_coupling(tddft_ctx* ctx, const double* X, double* BX, int nvec, int mode);
+
 /* Counters of the last tddft_apply_liouville call (for benchmarks): kernels launched, unique pair potentials
  * tau_vv' formed, and the milliseconds each stage took if timing was enabled. */
 typedef struct {
   long long kernel_launches;
   long long pair_ffts;
   double ms_total, ms_s1_to_real, ms_s23_hxc, ms_s4_pair_fft, ms_s5_contract, ms_s6_to_sphere, ms_s8_project;
+  double ms_s7_rotate_ace;  /* orbital rotations of Eq. 31 and the ACE term of D */
   int fft_batch; /* packed grids per FFT launch in use */
   int fft_path;  /* 0 = fused plane/x kernels, 1 = general pass kernels */
   int pair_batch; /* orbital pairs per launch of the pair-FFT pipeline in the last apply (<= 2*fft_batch) */
   int pair_tile;  /* tile edge of the last apply */
+  int k_chunk;    /* trial vectors processed together (< nvec: the pair potentials were recomputed per chunk) */
+  int blocks_resident; /* 1: the real-space functions of all spin blocks were resident; 0: one spin block at a time */
 } tddft_stats;
 int tddft_set_timing(tddft_ctx* ctx, int enabled); /* stage timing with CUDA events (adds synchronisation) */
 int tddft_get_stats(const tddft_ctx* ctx, tddft_stats* out);
@@ -146,6 +181,16 @@ int tddft_project(tddft_ctx* ctx, int spin, double* Y, long nfun);
 int tddft_gram(tddft_ctx* ctx, const double* V, const double* W, int m, long n_complex, double* G);
 /* real-space orbital phi_v of a spin on the FFT grid, DEVICE double [n1*n2*n3] out */
 int tddft_orbital_real_space(tddft_ctx* ctx, int spin, int v, double* out);
+/* Overlap function S_mn of Eq. 32 between the orbitals the exchange term runs on (rotated by
+ * wannier_u if given): S HOST double [nocc][nocc]. */
+int tddft_orbital_overlap(tddft_ctx* ctx, int spin, double* S);
+/* Exact exchange operator on nfun half-sphere functions of one spin (Eq. 28), VY = V_X Y brought back to
+ * the sphere: the (phi_occ, psi, phi_occ) operand pattern, nocc * nfun pair FFTs.  use_ace = 1 applies V_X^ACE of Eq. 29
+ * instead (needs options.ace).  Y, VY: DEVICE complex128 [nfun][npwh], VY must not alias Y.  No factor alpha. */
+int tddft_exchange_apply(tddft_ctx* ctx, int spin, const double* Y, double* VY, long nfun, int use_ace);
+/* FP64 peak probes for the roofline denominators (bench.py): register-resident DFMA and DMMA (mma.sync.m8n8k4.f64) loops on
+ * every SM, timed with CUDA events on the context's stream.  Both in TFLOP/s, HOST outputs. */
+int tddft_fp64_peak(tddft_ctx* ctx, double* dfma_tflops, double* dmma_tflops);
 
 const char* tddft_last_error(const tddft_ctx* ctx); /* ctx may be NULL: error of the last failed tddft_init */
 int tddft_destroy(tddft_ctx* ctx);

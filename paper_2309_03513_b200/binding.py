@@ -19,7 +19,8 @@ EXPORTS = [
     "tddft_enumerate_gvectors", "tddft_init", "tddft_npw_half", "tddft_gvectors", "tddft_vector_len",
     "tddft_workspace_bytes", "tddft_apply_liouville", "tddft_apply_liouville_host", "tddft_davidson",
     "tddft_set_timing", "tddft_get_stats", "tddft_pair_potentials", "tddft_project", "tddft_gram",
-    "tddft_orbital_real_space", "tddft_last_error", "tddft_destroy",
+    "tddft_orbital_real_space", "tddft_last_error", "tddft_destroy", "tddft_apply_coupling", "tddft_orbital_overlap",
+    "tddft_exchange_apply", "tddft_fp64_peak",
 ]
 
 
@@ -30,6 +31,12 @@ class tddft_options(C.Structure):
         ("workspace_gb", C.c_double), ("pair_tile", C.c_int), ("fft_batch", C.c_int),
         ("max_subspace", C.c_int), ("max_iter", C.c_int), ("tol", C.c_double),
         ("x0", C.c_void_p), ("n_x0", C.c_int), ("seed", C.c_ulonglong), ("fft_path", C.c_int),
+        ("block", C.c_int), ("precond", C.c_int), ("verbose", C.c_int),
+        ("sf_xc_kernel", C.c_int), ("sf_cut", C.c_double),
+        ("wannier_u_up", C.c_void_p), ("wannier_u_dn", C.c_void_p), ("s_thr", C.c_double),
+        ("pair_list_up", C.c_void_p), ("n_pairs_up", C.c_long), ("pair_list_dn", C.c_void_p), ("n_pairs_dn", C.c_long),
+        ("ace", C.c_int), ("psi_ace_up", C.c_void_p), ("n_ace_extra_up", C.c_int),
+        ("psi_ace_dn", C.c_void_p), ("n_ace_extra_dn", C.c_int),
     ]
 
 
@@ -37,7 +44,9 @@ class tddft_stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_longlong), ("pair_ffts", C.c_longlong), ("ms_total", C.c_double),
                 ("ms_s1_to_real", C.c_double), ("ms_s23_hxc", C.c_double), ("ms_s4_pair_fft", C.c_double),
                 ("ms_s5_contract", C.c_double), ("ms_s6_to_sphere", C.c_double), ("ms_s8_project", C.c_double),
-                ("fft_batch", C.c_int), ("fft_path", C.c_int), ("pair_batch", C.c_int), ("pair_tile", C.c_int)]
+                ("ms_s7_rotate_ace", C.c_double),
+                ("fft_batch", C.c_int), ("fft_path", C.c_int), ("pair_batch", C.c_int), ("pair_tile", C.c_int),
+                ("k_chunk", C.c_int), ("blocks_resident", C.c_int)]
 
 
 def load_library():
@@ -119,9 +128,24 @@ def tddft_init(lattice, grid, ecut_wfc_ry, nspin, nocc, psi_up, psi_dn, eig_up, 
     o.use_hartree_fxc = -1
     keep = [psi_up, psi_dn]
     for k, v in opt.items():
-        if k in ("vloc_up", "vloc_dn", "x0"):
+        if k in ("vloc_up", "vloc_dn", "x0", "psi_ace_up", "psi_ace_dn"):        # device tensors
             keep.append(v)
             setattr(o, k, None if v is None else v.data_ptr())
+            if k.startswith("psi_ace") and v is not None:
+                setattr(o, "n_ace_extra_" + k[-2:], int(v.shape[0]))
+        elif k in ("wannier_u_up", "wannier_u_dn"):                               # host matrices, read during init
+            if v is not None:
+                u = np.ascontiguousarray(v, dtype=np.float64)
+                keep.append(u)
+                setattr(o, k, u.ctypes.data)
+        elif k in ("pair_list_up", "pair_list_dn"):                               # host int pairs, read during init
+            if v is not None:
+                pl = np.ascontiguousarray(v, dtype=np.int32).reshape(-1, 2)
+                keep.append(pl)
+                setattr(o, k, pl.ctypes.data if len(pl) else np.zeros(2, dtype=np.int32).ctypes.data)
+                if not len(pl):
+                    keep.append(np.zeros(2, dtype=np.int32)); setattr(o, k, keep[-1].ctypes.data)
+                setattr(o, "n_pairs_" + k[-2:], len(pl))
         elif k == "cuda_stream":
             o.cuda_stream = v
         else:
@@ -209,6 +233,28 @@ def tddft_gram(ctx, V, W, m, n_complex):
 
 def tddft_orbital_real_space(ctx, spin, v, out):
     _check(_lib.tddft_orbital_real_space(ctx._h, C.c_int(spin), C.c_int(v), _ptr(out)), ctx._h)
+
+
+def tddft_apply_coupling(ctx, X, BX, nvec, mode=TDDFT_SPIN_CONSERVING):
+    """BX = (K2e - K2d) X; spin flip: X in the layout of the opposite flip direction (include/tddft.h)."""
+    _check(_lib.tddft_apply_coupling(ctx._h, _ptr(X), _ptr(BX), C.c_int(nvec), C.c_int(mode)), ctx._h)
+
+
+def tddft_orbital_overlap(ctx, spin, nocc):
+    S = np.zeros((nocc, nocc), dtype=np.float64)
+    _check(_lib.tddft_orbital_overlap(ctx._h, C.c_int(spin), S.ctypes.data_as(C.c_void_p)), ctx._h)
+    return S
+
+
+def tddft_exchange_apply(ctx, spin, Y, VY, nfun, use_ace=False):
+    _check(_lib.tddft_exchange_apply(ctx._h, C.c_int(spin), _ptr(Y), _ptr(VY), C.c_long(nfun), C.c_int(1 if use_ace else 0)), ctx._h)
+
+
+def tddft_fp64_peak(ctx):
+    """(DFMA TFLOP/s, DMMA TFLOP/s) measured on the context's device."""
+    a = C.c_double(0.0); b = C.c_double(0.0)
+    _check(_lib.tddft_fp64_peak(ctx._h, C.byref(a), C.byref(b)), ctx._h)
+    return a.value, b.value
 
 
 def tddft_last_error(ctx=None):

@@ -38,19 +38,15 @@ int ensure_arena(tddft_ctx* c, size_t bytes) {
 }
 
 // ---- stage timing ---------------------------------------------------------------------------------
-enum { ST_S1 = 0, ST_S23, ST_S4, ST_S5, ST_S6, ST_S8, ST_COUNT };
-struct StageTimer {
-    tddft_ctx* c; int idx = -1;
-    StageTimer(tddft_ctx* c_, int stage) : c(c_) {
-        if (!c->timing) return;
-        StageEvent ev; ev.stage = stage;
-        cudaEventCreate(&ev.beg); cudaEventCreate(&ev.end);
-        cudaEventRecord(ev.beg, c->stream);
-        c->events.push_back(ev); idx = (int)c->events.size() - 1;
-    }
-    ~StageTimer() { if (idx >= 0) cudaEventRecord(c->events[idx].end, c->stream); }
-};
-static void collect_timing(tddft_ctx* c) {
+StageTimer::StageTimer(tddft_ctx* c_, int stage) : c(c_) {
+    if (!c->timing) return;
+    StageEvent ev; ev.stage = stage;
+    cudaEventCreate(&ev.beg); cudaEventCreate(&ev.end);
+    cudaEventRecord(ev.beg, c->stream);
+    c->events.push_back(ev); idx = (int)c->events.size() - 1;
+}
+StageTimer::~StageTimer() { if (idx >= 0) cudaEventRecord(c->events[idx].end, c->stream); }
+void collect_timing(tddft_ctx* c) {
     if (!c->timing) return;
     cudaStreamSynchronize(c->stream);
     double ms[ST_COUNT] = {0};
@@ -62,6 +58,7 @@ static void collect_timing(tddft_ctx* c) {
     c->events.clear();
     c->stats.ms_s1_to_real = ms[ST_S1]; c->stats.ms_s23_hxc = ms[ST_S23]; c->stats.ms_s4_pair_fft = ms[ST_S4];
     c->stats.ms_s5_contract = ms[ST_S5]; c->stats.ms_s6_to_sphere = ms[ST_S6]; c->stats.ms_s8_project = ms[ST_S8];
+    c->stats.ms_s7_rotate_ace = ms[ST_S7X];
     c->stats.ms_total = 0; for (int i = 0; i < ST_COUNT; ++i) c->stats.ms_total += ms[i];
 }
 
@@ -114,20 +111,19 @@ static int leg_inverse_yz(tddft_ctx* c, const ZArgs& z) {
     c->stats.kernel_launches += 2;
     return TDDFT_OK;
 }
-#define TD_RC(call) do { int rc_ = (call); if (rc_) return rc_; } while (0)
 
-// tau_p = C[phi_i phi_j] for npairs pairs (device list), two pairs per complex grid
-// d_slots (optional): tau slot of each pair; null = slot p for pair p.  batch_pairs <= 2*fft_batch pairs per launch.
-static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pairs, const int* d_slots, long npairs, int batch_pairs, double* tau, int chunked) {
-    const long nr = c->hp.nr;
+// tau_p = C[A1[x_p] A2[y_p]] for npairs pairs (device list), two pairs per complex grid.
+// d_slots (optional): slot of each pair inside a batch of stot functions; null = slot p.  batch_pairs <= 2*fft_batch pairs per launch.
+int pair_potentials_dev(tddft_ctx* c, const double* A1, const double* A2, const int2* d_pairs, const int* d_slots, long npairs,
+                        int batch_pairs, double* tau, int chunked, long stot) {
     for (long p0 = 0; p0 < npairs; p0 += batch_pairs) {
         const int np = (int)std::min<long>(batch_pairs, npairs - p0);
         const int nb = (np + 1) / 2;
         ZArgs z = zpass_args(c, nb, KIND_PROD);
-        z.phi = phi; z.pairs = d_pairs + p0; z.npairs = np;
+        z.phi = A1; z.phi2 = A2; z.pairs = d_pairs + p0; z.npairs = np;
         TD_RC(leg_forward_yz(c, ZL_PAIR, z));
         TD_RC(leg_x(c, SM_CONV, nb, KIND_PROD));
-        z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = d_slots ? 0 : p0; z.ftotal = npairs;
+        z.dst = tau; z.nfun = np; z.sscale = 1.0; z.chunked = chunked; z.fbase = d_slots ? 0 : p0; z.ftotal = stot;
         z.slots = d_slots ? d_slots + p0 : nullptr;
         TD_RC(leg_inverse_yz(c, z));
         c->stats.pair_ffts += np;
@@ -136,8 +132,7 @@ static int pair_potentials_dev(tddft_ctx* c, const double* phi, const int2* d_pa
 }
 
 // S1: nfun half-sphere functions -> real space, dst[f][r] = Omega^-1/2 sum_G c_f(G) exp(i G.r)
-static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked) {
-    const long nr = c->hp.nr;
+int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked) {
     const double scale = 1.0 / std::sqrt(c->hp.omega);
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
@@ -152,8 +147,8 @@ static int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, d
     return TDDFT_OK;
 }
 
-// S6+S7: real-space functions -> half sphere, AX = (Omega^1/2/N_r) FFT[src] + (|G|^2/2 - eps_v) X
-static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig) {
+// S6+S7: real-space functions (chunked batch) -> half sphere, AX = (Omega^1/2/N_r) FFT[src] + (|G|^2/2 - eps_v) X; X = null: no D term
+int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig) {
     const long nr = c->hp.nr;
     const double scale = std::sqrt(c->hp.omega) / (double)nr;
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
@@ -170,8 +165,7 @@ static int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cpl
 }
 
 // S3 Hartree part: vh[kk] = C[scale * (d0[kk] + d1[kk])]
-static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scale, int kc, double* vh) {
-    const long nr = c->hp.nr;
+int hartree(tddft_ctx* c, const double* d0, const double* d1, double scale, int kc, double* vh) {
     for (int f0 = 0; f0 < kc; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, kc - f0);
         const int nb = (nf + 1) / 2;
@@ -185,10 +179,11 @@ static int hartree(tddft_ctx* c, const double* d0, const double* d1, double scal
     return TDDFT_OK;
 }
 
-// S8: rows <- P_c rows with the occupied orbitals of tgt_spin, two tensor-core GEMMs
-int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_stride, double* O, size_t o_cap) {
+// Yout[row] += scale * sum_u basis_u <basis_u|Yin[row]>: two tensor-core GEMMs (S8: P_c of PAPER.md:105; ACE term of D, Eq. 29)
+int lowrank_rows(tddft_ctx* c, const double* basis, int nb_, const double* Yin, double* Yout, int nrows, int grp, long grp_stride,
+                 double scale, double* O, size_t o_cap) {
     const long k2 = 2 * c->hp.npwh;
-    const int no = c->nocc[tgt];
+    const int no = nb_;
     const long ldo = (nrows + 1) & ~1L;                      // even pitch: 16-byte aligned rows for the async copies
     // k splits chosen so that the CTAs fill whole waves of the SMs (ordered reduction, deterministic)
     const long tiles = gemm_nt_tile_count(no, nrows);
@@ -199,11 +194,15 @@ int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_
         const double eff = (double)ctas / (double)(waves * c->num_sms);
         if (eff > best + 0.02) { best = eff; splits = s; }
     }
+    if ((size_t)no * ldo > o_cap) return set_err(c, TDDFT_ENOMEM, "projector scratch too small");
     double* partial = splits > 1 ? O + (size_t)no * ldo : nullptr;
-    TD_CUDA(c, launch_gemm_nt(c->psi[tgt], k2, Y, k2, grp, grp_stride, O, ldo, no, nrows, k2, k2, 2.0, splits, partial, c->stream));
-    TD_CUDA(c, launch_gemm_tn_acc(O, ldo, c->psi[tgt], k2, Y, k2, grp, grp_stride, nrows, k2, no, -1.0, c->stream));
+    TD_CUDA(c, launch_gemm_nt(basis, k2, Yin, k2, grp, grp_stride, O, ldo, no, nrows, k2, k2, 2.0, splits, partial, c->stream));
+    TD_CUDA(c, launch_gemm_tn_acc(O, ldo, basis, k2, Yout, k2, grp, grp_stride, nrows, k2, no, scale, c->stream));
     c->stats.kernel_launches += 2 + (splits > 1 ? 1 : 0);
     return TDDFT_OK;
+}
+int project_rows(tddft_ctx* c, int tgt, double* Y, int nrows, int grp, long grp_stride, double* O, size_t o_cap) {
+    return lowrank_rows(c, c->psi[tgt], c->nocc[tgt], Y, Y, nrows, grp, grp_stride, -1.0, O, o_cap);
 }
 size_t project_scratch_doubles(const tddft_ctx* c, int maxocc, int nrows, size_t max_bytes) {
     const size_t one = (size_t)maxocc * ((nrows + 1) & ~1L);
@@ -211,6 +210,50 @@ size_t project_scratch_doubles(const tddft_ctx* c, int maxocc, int nrows, size_t
     int mult = 13;
     while (mult > 1 && one * mult > cap) --mult;
     return one * mult;
+}
+
+// ---- real-space orbitals ------------------------------------------------------------------------------
+// d_phi[s] <- phi_vs(r), or the rotated phi~_n = sum_v U[v][n] phi_v of Eq. 31 when wannier_u was given (rotation done in the sphere)
+static int compute_phi(tddft_ctx* c, int s) {
+    const long npwh = c->hp.npwh;
+    const int N = c->nocc[s];
+    FunLayout lay{0, 0, npwh, 1, 0};
+    if (!c->d_U[s]) return to_real_space(c, (const cplx*)c->psi[s], lay, N, c->d_phi[s], 0);
+    double* rot = nullptr;
+    if (cudaMalloc((void**)&rot, sizeof(cplx) * (size_t)N * npwh) != cudaSuccess) { cudaGetLastError(); return set_err(c, TDDFT_ENOMEM, "rotated orbitals: allocation failed"); }
+    cudaError_t e = cudaMemsetAsync(rot, 0, sizeof(cplx) * (size_t)N * npwh, c->stream);
+    if (e == cudaSuccess) e = launch_gemm_tn_acc(c->d_U[s], N, c->psi[s], 2 * npwh, rot, 2 * npwh, N, 0, N, 2 * npwh, N, 1.0, c->stream);
+    int rc = e == cudaSuccess ? to_real_space(c, (const cplx*)rot, lay, N, c->d_phi[s], 0) : set_err(c, TDDFT_ECUDA, cudaGetErrorString(e));
+    cudaStreamSynchronize(c->stream);
+    cudaFree(rot);
+    return rc;
+}
+int ensure_phi(tddft_ctx* c, int s) {
+    if (!c->phi_shared || c->phi_spin == s) return TDDFT_OK;
+    c->phi_spin = -1;
+    TD_RC(compute_phi(c, s));
+    c->phi_spin = s;
+    return TDDFT_OK;
+}
+// S_mn of Eq. 32 for the exchange orbitals of spin s, HOST S [N][N]
+int orbital_overlap(tddft_ctx* c, int s, double* S) {
+    const long nr = c->hp.nr;
+    const int N = c->nocc[s];
+    TD_RC(ensure_phi(c, s));
+    double* sq = nullptr;
+    const int splits = (int)std::max<long>(1, std::min<long>(64, nr / 16384));
+    if (cudaMalloc((void**)&sq, sizeof(double) * ((size_t)N * nr + (size_t)N * N * (splits + 1))) != cudaSuccess) { cudaGetLastError(); return set_err(c, TDDFT_ENOMEM, "overlap: allocation failed"); }
+    double* Sd = sq + (size_t)N * nr; double* part = Sd + (size_t)N * N;
+    cudaError_t e = launch_square(c->d_phi[s], (long)N * nr, sq, c->stream);
+    if (e == cudaSuccess) e = launch_gemm_nt(sq, nr, sq, nr, N, 0, Sd, N, N, N, nr, 0, 1.0, splits, part, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S, Sd, sizeof(double) * N * N, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(sq);
+    if (e != cudaSuccess) return set_err(c, TDDFT_ECUDA, std::string("overlap: ") + cudaGetErrorString(e));
+    std::vector<double> d(N);
+    for (int m = 0; m < N; ++m) d[m] = std::sqrt(S[(size_t)m * N + m]);
+    for (int m = 0; m < N; ++m) for (int n = 0; n < N; ++n) S[(size_t)m * N + n] /= d[m] * d[n];
+    return TDDFT_OK;
 }
 
 // ---- pair tiles -------------------------------------------------------------------------------------
@@ -225,12 +268,11 @@ static void choose_subblock(int cap, int* si_out, int* sj_out) {
             if (cost < best) { best = cost; *si_out = si; *sj_out = sj; }
         }
 }
-static int build_tiles(tddft_ctx* c, int spin, int T) {
+int build_tiles(tddft_ctx* c, int spin, int T) {
     PairTiles& pt = c->tiles[spin];
     const int N = c->nocc[spin];
     if (pt.T == T && pt.nocc == N && pt.d_pairs) return TDDFT_OK;
     if (pt.d_pairs) cudaFree(pt.d_pairs);
-    if (pt.d_slot) cudaFree(pt.d_slot);
     if (pt.d_pslot) cudaFree(pt.d_pslot);
     pt = PairTiles{};
     pt.T = T; pt.nocc = N;
@@ -239,48 +281,66 @@ static int build_tiles(tddft_ctx* c, int spin, int T) {
     // pairs packed into one complex grid still share their first orbital.
     choose_subblock(2 * c->fft_batch, &pt.sbi, &pt.sbj);
     pt.batch_pairs = pt.sbi * pt.sbj;
+    const std::vector<char>& mask = c->mask[spin];      // near-sightedness truncation (Eq. 32 / explicit pair list); empty = all pairs
     const int nb = (N + T - 1) / T;
-    std::vector<int2> pairs; std::vector<int> slot, pslot;
+    std::vector<int2> pairs; std::vector<int> pslot;
     for (int bi = 0; bi < nb; ++bi)
         for (int bj = bi; bj < nb; ++bj) {
             TileInfo t{};
             t.i0 = bi * T; t.ti = std::min(T, N - t.i0); t.j0 = bj * T; t.tj = std::min(T, N - t.j0);
-            t.pair_off = (long)pairs.size(); t.slot_off = (long)slot.size();
-            std::vector<int> s((size_t)t.ti * t.tj, -1);
+            t.diag = bi == bj;
+            t.pair_off = (long)pairs.size();
+            // tau slots (the contraction's layout): dense i*tj + j, or the packed upper triangle i(2 tj - i + 1)/2 + (j - i) on the diagonal
+            auto slot_of = [&](int i, int j) { return t.diag ? i * (2 * t.tj - i + 1) / 2 + (j - i) : i * t.tj + j; };
+            t.nslots = t.diag ? (long)t.ti * (t.ti + 1) / 2 : (long)t.ti * t.tj;
             int cnt = 0;
-            for (int i = 0; i < t.ti; ++i)
-                for (int j = 0; j < t.tj; ++j) {
-                    const int gi = t.i0 + i, gj = t.j0 + j;
-                    if (gi > gj) continue;
-                    s[(size_t)i * t.tj + j] = cnt++;     // tau slots stay row-major (the contraction's layout)
-                }
             for (int si0 = 0; si0 < t.ti; si0 += pt.sbi)
                 for (int sj0 = 0; sj0 < t.tj; sj0 += pt.sbj)
                     for (int i = si0; i < std::min(si0 + pt.sbi, t.ti); ++i)
                         for (int j = sj0; j < std::min(sj0 + pt.sbj, t.tj); ++j) {
                             const int gi = t.i0 + i, gj = t.j0 + j;
                             if (gi > gj) continue;
+                            if (!mask.empty() && !mask[(size_t)gi * N + gj]) continue;
                             pairs.push_back(make_int2(gi, gj));
-                            pslot.push_back(s[(size_t)i * t.tj + j]);
+                            pslot.push_back(slot_of(i, j));
+                            ++cnt;
                         }
-            if (bi == bj) for (int i = 0; i < t.ti; ++i) for (int j = 0; j < i; ++j) s[(size_t)i * t.tj + j] = s[(size_t)j * t.tj + i];
             t.npairs = cnt;
-            slot.insert(slot.end(), s.begin(), s.end());
-            t.slotT_off = -1;
-            if (bi != bj) {
-                t.slotT_off = (long)slot.size();
-                for (int j = 0; j < t.tj; ++j) for (int i = 0; i < t.ti; ++i) slot.push_back(s[(size_t)i * t.tj + j]);
-            }
+            t.partial = cnt < t.nslots;
             pt.max_pairs = std::max<long>(pt.max_pairs, cnt);
+            pt.total_pairs += cnt;
             pt.tiles.push_back(t);
         }
-    TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * pairs.size()));
-    TD_CUDA(c, cudaMalloc((void**)&pt.d_slot, sizeof(int) * slot.size()));
-    TD_CUDA(c, cudaMalloc((void**)&pt.d_pslot, sizeof(int) * pslot.size()));
+    const size_t np = std::max<size_t>(pairs.size(), 1);
+    TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * np));
+    TD_CUDA(c, cudaMalloc((void**)&pt.d_pslot, sizeof(int) * np));
     TD_CUDA(c, cudaMemcpyAsync(pt.d_pslot, pslot.data(), sizeof(int) * pslot.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaMemcpyAsync(pt.d_pairs, pairs.data(), sizeof(int2) * pairs.size(), cudaMemcpyHostToDevice, c->stream));
-    TD_CUDA(c, cudaMemcpyAsync(pt.d_slot, slot.data(), sizeof(int) * slot.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors go out of scope
+    return TDDFT_OK;
+}
+
+size_t workspace_budget(const tddft_ctx* c) {
+    size_t fr = 0, tot = 0; cudaMemGetInfo(&fr, &tot);
+    size_t budget = (size_t)(0.85 * (double)(fr + c->arena_bytes));
+    if (c->workspace_gb > 0) budget = std::min(budget, (size_t)(c->workspace_gb * 1073741824.0));
+    return budget;
+}
+
+// ---- orbital rotation of Eq. 31 in the sphere: dst_n = sum_v U[v][n] src_v for each of kc trial vectors ------
+// src rows of trial vector kk at src + kk*src_vstride (doubles), dst likewise; rows are 2*npwh doubles apart.  accumulate = false
+// zeroes dst first.  Ut = false uses U[v][n] (to the rotated basis), true uses U^T (back to the canonical basis).
+static int rotate_rows(tddft_ctx* c, int spin, bool back, const double* src, long src_vstride, double* dst, long dst_vstride, int kc,
+                       bool accumulate) {
+    const int N = c->nocc[spin];
+    const long k2 = 2 * c->hp.npwh;
+    const double* At = back ? c->d_Ut[spin] : c->d_U[spin];     // At[k][m]: forward k = v, m = n: U[v][n]; back k = n, m = v: U^T[n][v]
+    for (int kk = 0; kk < kc; ++kk) {
+        double* d = dst + (long)kk * dst_vstride;
+        if (!accumulate) TD_CUDA(c, cudaMemsetAsync(d, 0, sizeof(double) * k2 * N, c->stream));
+        TD_CUDA(c, launch_gemm_tn_acc(At, N, src + (long)kk * src_vstride, k2, d, k2, N, 0, N, k2, N, 1.0, c->stream));
+        c->stats.kernel_launches += 1;
+    }
     return TDDFT_OK;
 }
 
@@ -293,65 +353,101 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     if (Xd == AXd) return set_err(c, TDDFT_EINVAL, "apply: AX must not alias X");
     if (mode < 0 || mode > 2) return set_err(c, TDDFT_EINVAL, "apply: unknown mode");
     if (mode != TDDFT_SPIN_CONSERVING && c->nspin != 2) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    TD_CUDA(c, cudaSetDevice(c->device));
     const cplx* X = (const cplx*)Xd; cplx* AX = (cplx*)AXd;
     const long nr = c->hp.nr, npwh = c->hp.npwh, L = vector_len(c, mode);
     c->stats = tddft_stats{};
     std::vector<Block> blocks;
     if (mode == TDDFT_SPIN_CONSERVING) { long off = 0; for (int s = 0; s < c->nspin; ++s) { blocks.push_back({s, s, off}); off += (long)c->nocc[s] * npwh; } }
     else { const int src = (mode == TDDFT_SPIN_FLIP) ? 0 : 1; blocks.push_back({src, 1 - src, 0}); }
+    const int nblk = (int)blocks.size();
     const bool hxc = (mode == TDDFT_SPIN_CONSERVING) && c->use_hartree_fxc;
-    int maxocc = 0, sumocc = 0;
-    for (auto& b : blocks) { maxocc = std::max(maxocc, std::max(c->nocc[b.src], c->nocc[b.tgt])); sumocc += c->nocc[b.src]; }
-
-    // ---- workspace plan: k chunk kc and tile edge T under the budget --------------------------------
-    size_t budget;
-    {
-        size_t fr = 0, tot = 0; cudaMemGetInfo(&fr, &tot);
-        budget = (size_t)(0.85 * (double)(fr + c->arena_bytes));
-        if (c->workspace_gb > 0) budget = std::min(budget, (size_t)(c->workspace_gb * 1073741824.0));
+    const bool sfk = (mode != TDDFT_SPIN_CONSERVING) && c->sf_xc;        // K1e^SF of Eq. 24 with the kernel of Eq. 26
+    int maxocc = 0, sumsrc = 0, maxsrc = 0, maxbasis = 0;
+    bool rot = false;
+    for (auto& b : blocks) {
+        maxocc = std::max(maxocc, std::max(c->nocc[b.src], c->nocc[b.tgt])); sumsrc += c->nocc[b.src]; maxsrc = std::max(maxsrc, c->nocc[b.src]);
+        maxbasis = std::max(maxbasis, std::max(c->nocc[b.tgt], c->n_ace[b.tgt]));
+        rot = rot || c->d_U[b.src];
     }
-    int kc = nvec, T = 0;
-    size_t fixed = 0;
+
+    // ---- workspace plan: all spin blocks resident or one at a time, k chunk kc and tile edge T under the budget ----------------
+    const size_t budget = workspace_budget(c);
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
+    const int tcap = contract_full_max_tile();
+    int kc = nvec, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
+    auto fixed_bytes = [&](int kc_, bool res) {
+        size_t f = grid_b * (size_t)kc_ * ((size_t)(res ? sumsrc : maxsrc) + (size_t)maxsrc);
+        if (hxc) f += grid_b * (size_t)kc_ * (2 * nblk + 1);
+        if (sfk) f += grid_b * (size_t)kc_ * 2;
+        if (rot) f += 2 * sizeof(cplx) * (size_t)kc_ * maxsrc * npwh;
+        return f + sizeof(double) * project_scratch_doubles(c, maxbasis, kc_ * maxsrc, budget) + 8192;
+    };
     for (;;) {
-        fixed = grid_b * (size_t)kc * ((size_t)sumocc + (size_t)maxocc + (hxc ? 2 * blocks.size() + 1 : 0))
-              + sizeof(double) * project_scratch_doubles(c, maxocc, kc * maxocc, budget) + 4096;
-        const int tcap = c->ct_full ? contract_full_max_tile() : 128;
-        T = std::min(std::min(maxocc, tcap), c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tcap);
-        const int tmin = std::min(maxocc, 16);
-        while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 8);
-        if (fixed + grid_b * (size_t)T * T <= budget) break;
+        fixed = fixed_bytes(kc, resident);
+        T = std::min(std::min(maxsrc, tcap), c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tcap);
+        const int tmin = std::min(maxsrc, 16);
+        while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 4);
+        const bool fits = fixed + grid_b * (size_t)T * T <= budget;
+        // a small tile costs a(r)/out(r) traffic in S5: before shrinking T below half its cap, give up residency of all blocks
+        if (fits && (T >= std::min(maxsrc, tcap / 2) || (!resident || nblk == 1) )) break;
+        if (resident && nblk > 1) { resident = false; continue; }
+        if (fits) break;
         if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
         kc = (kc + 1) / 2;
     }
-    if (c->ct_full) { const int nbk = (maxocc + T - 1) / T; T = (maxocc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
-    else if (T >= 32) T &= ~31;   // the row-block contraction gives each warp 32 rows of a tile
+    if (nblk == 1) resident = true;
+    { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
     int rc = ensure_arena(c, fixed + grid_b * (size_t)T * T);
     if (rc) return rc;
     char* p = c->arena;
     auto carve = [&](size_t bytes) { char* q = p; p += (bytes + 255) / 256 * 256; return (double*)q; };
-    std::vector<double*> a(blocks.size());
-    for (size_t b = 0; b < blocks.size(); ++b) a[b] = carve(grid_b * (size_t)kc * c->nocc[blocks[b].src]);
-    double* out = carve(grid_b * (size_t)kc * maxocc);
-    std::vector<double*> drho(blocks.size(), nullptr), V(blocks.size(), nullptr);
+    std::vector<double*> a(nblk);
+    if (resident) for (int b = 0; b < nblk; ++b) a[b] = carve(grid_b * (size_t)kc * c->nocc[blocks[b].src]);
+    else { double* a0 = carve(grid_b * (size_t)kc * maxsrc); for (int b = 0; b < nblk; ++b) a[b] = a0; }
+    double* out = carve(grid_b * (size_t)kc * maxsrc);
+    std::vector<double*> drho(nblk, nullptr), V(nblk, nullptr);
     double* vh = nullptr;
-    if (hxc) { for (size_t b = 0; b < blocks.size(); ++b) { drho[b] = carve(grid_b * kc); V[b] = carve(grid_b * kc); } vh = carve(grid_b * kc); }
-    const size_t o_cap = project_scratch_doubles(c, maxocc, kc * maxocc, budget);
+    if (hxc) { for (int b = 0; b < nblk; ++b) { drho[b] = carve(grid_b * kc); V[b] = carve(grid_b * kc); } vh = carve(grid_b * kc); }
+    if (sfk) { drho[0] = carve(grid_b * kc); V[0] = carve(grid_b * kc); }
+    cplx *Xr = nullptr, *Yr = nullptr;
+    if (rot) { Xr = (cplx*)carve(sizeof(cplx) * (size_t)kc * maxsrc * npwh); Yr = (cplx*)carve(sizeof(cplx) * (size_t)kc * maxsrc * npwh); }
+    const size_t o_cap = project_scratch_doubles(c, maxbasis, kc * maxsrc, budget);
     double* O = carve(sizeof(double) * o_cap);
     double* tau = carve(grid_b * (size_t)T * T);
     for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src])); if (rc) return rc; }
-    c->last_pair_tile = T; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs;
+    c->last_pair_tile = T; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = kc; c->last_resident = resident ? 1 : 0;
 
     for (int k0 = 0; k0 < nvec; k0 += kc) {
         const int kcc = std::min(kc, nvec - k0);
-        // S1 (+S2): trial functions to real space, response densities
-        for (size_t b = 0; b < blocks.size(); ++b) {
-            const int no = c->nocc[blocks[b].src];
-            FunLayout lay{L, blocks[b].off, npwh, kcc, k0};
+        int loaded = -1;                                   // block whose a(r) sits in the shared buffer (non-resident plan)
+        // S1: trial functions of block b to real space (rotated to the localized orbitals first if wannier_u was given)
+        auto load_block = [&](int b) -> int {
+            const Block& bl = blocks[b];
+            const int no = c->nocc[bl.src];
             if (c->overlap_copies) TD_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_x_ready[b], 0));     // this block of X has arrived
-            { StageTimer t(c, ST_S1); rc = to_real_space(c, X, lay, no * kcc, a[b], 1); if (rc) return rc; }
-            if (hxc) { StageTimer t(c, ST_S23); TD_CUDA(c, launch_drho(c->d_phi[blocks[b].src], a[b], no, kcc, nr, drho[b], c->stream)); c->stats.kernel_launches += (kcc + 3) / 4; }
-        }
+            TD_RC(ensure_phi(c, bl.src));
+            FunLayout lay{L, bl.off, npwh, kcc, k0};
+            const cplx* src = X;
+            if (c->d_U[bl.src]) {
+                StageTimer t(c, ST_S7X);
+                TD_RC(rotate_rows(c, bl.src, false, (const double*)(X + (long)k0 * L + bl.off), 2 * L, (double*)Xr, 2L * no * npwh, kcc, false));
+                lay = FunLayout{(long)no * npwh, 0, npwh, kcc, 0}; src = Xr;
+            }
+            StageTimer t(c, ST_S1);
+            TD_RC(to_real_space(c, src, lay, no * kcc, a[b], 1));
+            loaded = b;
+            return TDDFT_OK;
+        };
+        auto response_density = [&](int b) -> int {      // S2: drho = sum_v phi_v a_v (Eq. 4 inner sum; Eq. 22 for spin flip)
+            StageTimer t(c, ST_S23);
+            const Block& bl = blocks[b];
+            TD_CUDA(c, launch_drho(c->d_phi[bl.src], a[b], c->nocc[bl.src], kcc, nr, drho[b], c->stream));
+            c->stats.kernel_launches += (kcc + 3) / 4;
+            return TDDFT_OK;
+        };
+        if (resident) for (int b = 0; b < nblk; ++b) { TD_RC(load_block(b)); if (hxc || sfk) TD_RC(response_density(b)); }
+        else if (hxc) for (int b = 0; b < nblk; ++b) { TD_RC(load_block(b)); TD_RC(response_density(b)); }
         // S3: Hartree + f_xc potential (Eq. 4 with f_Hxc = v_c + f_xc)
         if (hxc) {
             StageTimer t(c, ST_S23);
@@ -366,28 +462,49 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
                 c->stats.kernel_launches += 1;
             }
         }
-        for (size_t b = 0; b < blocks.size(); ++b) {
+        for (int b = 0; b < nblk; ++b) {
             const Block& bl = blocks[b];
             const int no = c->nocc[bl.src];
+            if (!resident && loaded != b) TD_RC(load_block(b));
+            TD_RC(ensure_phi(c, bl.src));
             const double* phi = c->d_phi[bl.src];
+            if (sfk) {   // K1e^SF: V = f^SF drho^SF (Eq. 24)
+                if (!resident) TD_RC(response_density(b));
+                StageTimer t(c, ST_S23);
+                TD_CUDA(c, launch_scale_potential(c->d_fsf, drho[b], kcc, nr, V[b], c->stream)); c->stats.kernel_launches += 1;
+            }
             { StageTimer t(c, ST_S5);
-              TD_CUDA(c, launch_out_init(phi, hxc ? V[b] : nullptr, c->vloc[bl.tgt], a[b], no, kcc, nr, out, c->stream)); c->stats.kernel_launches += 1; }
+              TD_CUDA(c, launch_out_init(phi, (hxc || sfk) ? V[b] : nullptr, c->vloc[bl.tgt], a[b], no, kcc, nr, out, c->stream)); c->stats.kernel_launches += 1; }
             // S4 + S5: exact-exchange response, tile by tile (Eq. 6; tau_vv' of PAPER.md:230)
             if (c->alpha != 0.0) {
                 const PairTiles& pt = c->tiles[bl.src];
                 for (const TileInfo& t : pt.tiles) {
-                    { StageTimer tm(c, ST_S4); rc = pair_potentials_dev(c, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1); if (rc) return rc; }
+                    if (t.npairs == 0) continue;            // every pair of the tile was truncated
+                    { StageTimer tm(c, ST_S4);
+                      if (t.partial) TD_CUDA(c, cudaMemsetAsync(tau, 0, grid_b * (size_t)t.nslots, c->stream));
+                      rc = pair_potentials_dev(c, phi, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1, t.nslots); if (rc) return rc; }
                     StageTimer tm(c, ST_S5);
-                    if (c->ct_full) TD_CUDA(c, launch_contract_full(t.slotT_off < 0, out, a[b], tau, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc,
-                                                                   t.slotT_off < 0 ? (long)t.npairs : (long)t.ti * t.tj, nr, c->alpha, c->stream));
-                    else if (t.slotT_off >= 0) TD_CUDA(c, launch_contract_dual(out, a[b], tau, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, nr, c->alpha, c->stream));
-                    else TD_CUDA(c, launch_contract_single(out, a[b], tau, pt.d_slot + t.slot_off, c->d_zeros, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, t.npairs, nr, c->alpha, c->stream));
+                    TD_CUDA(c, launch_contract_full(t.diag, out, a[b], tau, t.i0, t.ti, t.j0, t.tj, kcc, (long)no * kcc, t.nslots, nr, c->alpha, c->stream));
                     c->stats.kernel_launches += (kcc + 15) / 16;
                 }
             }
             // S6 + S7: back to the sphere, add D (Eq. 3 with the model H of reading A4)
             FunLayout lay{L, bl.off, npwh, kcc, k0};
-            { StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, X, AX, lay, c->d_eig[bl.src]); if (rc) return rc; }
+            if (c->d_U[bl.src]) {       // Eq. 31: the grid part was computed for the rotated functions, rotate it back and add D
+                FunLayout layr{(long)no * npwh, 0, npwh, kcc, 0};
+                { StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, nullptr, Yr, layr, nullptr); if (rc) return rc; }
+                StageTimer t(c, ST_S7X);
+                TD_CUDA(c, launch_d_term(X, AX, lay, no * kcc, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1;
+                TD_RC(rotate_rows(c, bl.src, true, (const double*)Yr, 2L * no * npwh, (double*)(AX + (long)k0 * L + bl.off), 2 * L, kcc, true));
+            } else {
+                StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, X, AX, lay, c->d_eig[bl.src]); if (rc) return rc;
+            }
+            if (c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {   // H includes alpha V_X^ACE (Eqs. 28-30)
+                StageTimer t(c, ST_S7X);
+                rc = lowrank_rows(c, (const double*)c->d_xi[bl.tgt], c->n_ace[bl.tgt], (const double*)(X + (long)k0 * L + bl.off),
+                                  (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, -c->alpha, O, o_cap);
+                if (rc) return rc;
+            }
             // S8: conduction-band projector of the target spin
             { StageTimer t(c, ST_S8);
               rc = project_rows(c, bl.tgt, (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, O, o_cap); if (rc) return rc; }
@@ -420,13 +537,15 @@ int tddft_enumerate_gvectors(const double* lattice, double ecut, long capacity, 
 int tddft_destroy(tddft_ctx* c) {
     if (!c) return TDDFT_OK;
     cudaFree(c->d_idx_p); cudaFree(c->d_idx_m); cudaFree(c->d_kin); cudaFree(c->d_vc); cudaFree(c->d_cmap[0]); cudaFree(c->d_cmap[1]);
-    for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_phi[s]); }
+    cudaSetDevice(c->device);
+    cudaFree(c->d_phi[0]); if (!c->phi_shared) cudaFree(c->d_phi[1]);
+    for (int s = 0; s < 2; ++s) { cudaFree(c->d_eig[s]); cudaFree(c->d_U[s]); cudaFree(c->d_Ut[s]); cudaFree(c->d_xi[s]); }
     for (int a = 0; a < 3; ++a) { cudaFree(c->d_tw[a]); cudaFree(c->d_fxc[a]); }
-    cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_zeros);
+    cudaFree(c->d_work); cudaFree(c->arena); cudaFree(c->d_fsf);
     cudaFree(c->host_dx); cudaFree(c->host_dax);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (int i = 0; i < 2; ++i) { if (c->ev_x_ready[i]) cudaEventDestroy(c->ev_x_ready[i]); if (c->ev_ax_done[i]) cudaEventDestroy(c->ev_ax_done[i]); }
-    for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_slot); cudaFree(c->tiles[s].d_pslot); }
+    for (int s = 0; s < 2; ++s) { cudaFree(c->tiles[s].d_pairs); cudaFree(c->tiles[s].d_pslot); }
     cudaGetLastError();
     delete c;
     return TDDFT_OK;
@@ -453,7 +572,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         const char* perr = build_host_plan(lattice, grid, ecut, &c->hp);
         if (perr) return fail(std::strstr(perr, "plan") ? TDDFT_EUNSUPPORTED : TDDFT_EINVAL, std::string("init: ") + perr);
         c->ecut = ecut; c->alpha = alpha; c->nspin = nspin;
-        { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev); if (c->num_sms < 1) c->num_sms = 148; }
+        { int dev = 0; cudaGetDevice(&dev); c->device = dev; cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev); if (c->num_sms < 1) c->num_sms = 148; }
         c->nocc[0] = nocc[0]; c->nocc[1] = nspin == 2 ? nocc[1] : 0;
         c->psi[0] = psi_up; c->psi[1] = nspin == 2 ? psi_dn : nullptr;
         c->eig_h[0].assign(eig_up, eig_up + nocc[0]);
@@ -467,10 +586,16 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->workspace_gb = opt->workspace_gb; c->pair_tile = opt->pair_tile; c->fft_batch = opt->fft_batch;
             c->dav_max_subspace = opt->max_subspace; c->dav_max_iter = opt->max_iter; c->dav_tol = opt->tol;
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
+            c->dav_block = opt->block; c->dav_precond = opt->precond; c->verbose = opt->verbose;
             c->fused = opt->fft_path == 0;
+            c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
+            if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");
+            if (opt->s_thr < 0 || opt->n_pairs_up < 0 || opt->n_pairs_dn < 0 || opt->n_ace_extra_up < 0 || opt->n_ace_extra_dn < 0)
+                return fail(TDDFT_EINVAL, "init: negative s_thr / pair count / ACE orbital count");
+            if ((opt->n_ace_extra_up > 0 && !opt->psi_ace_up) || (opt->n_ace_extra_dn > 0 && !opt->psi_ace_dn))
+                return fail(TDDFT_EINVAL, "init: n_ace_extra > 0 without psi_ace");
         } else c->fused = true;
         c->fused = c->fused && fused_supported(grid);
-        { const char* e = getenv("TDDFT_CT_FULL"); c->ct_full = !(e && atoi(e) == 0); }
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) {
             // large launches win (measured up to 192 grids): with the plane-major unit order the CTAs of a launch share orbital
@@ -500,8 +625,6 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             INIT_CUDA(cudaMemcpy(c->d_cmap[k], c->hp.colmap[k].data(), sizeof(int) * c->hp.colmap[k].size(), cudaMemcpyHostToDevice));
         }
         INIT_CUDA(cudaMalloc((void**)&c->d_work, sizeof(cplx) * nr * c->fft_batch));
-        INIT_CUDA(cudaMalloc((void**)&c->d_zeros, 1024));
-        INIT_CUDA(cudaMemset(c->d_zeros, 0, 1024));
         std::vector<double> kin(npwh);
         for (long g = 0; g < npwh; ++g) kin[g] = 0.5 * c->hp.g2[g];
         INIT_CUDA(cudaMemcpy(c->d_idx_p, idx_p_h.data(), sizeof(int) * npwh, cudaMemcpyHostToDevice));
@@ -518,24 +641,79 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             INIT_CUDA(cudaMalloc((void**)&c->d_tw[a], sizeof(cplx) * n));
             INIT_CUDA(cudaMemcpy(c->d_tw[a], tw.data(), sizeof(cplx) * n, cudaMemcpyHostToDevice));
         }
+        INIT_CUDA(cudaDeviceSynchronize());      // the table uploads above ran on the legacy stream; kernels below run on c->stream
         for (int s = 0; s < nspin; ++s) {
             INIT_CUDA(cudaMalloc((void**)&c->d_eig[s], sizeof(double) * c->nocc[s]));
             INIT_CUDA(cudaMemcpy(c->d_eig[s], c->eig_h[s].data(), sizeof(double) * c->nocc[s], cudaMemcpyHostToDevice));
-            INIT_CUDA(cudaMalloc((void**)&c->d_phi[s], sizeof(double) * nr * c->nocc[s]));
-            FunLayout lay{0, 0, npwh, 1, 0};
-            int rc = to_real_space(c, (const cplx*)c->psi[s], lay, c->nocc[s], c->d_phi[s], 0);
-            if (rc) { std::string m = c->err; return fail(rc, m); }
         }
-        // rho0 and LDA f_xc (Eq. 8)
+        // orbital rotation of Eq. 31: U and U^T on the device
+        for (int s = 0; s < nspin; ++s) {
+            const double* U = opt ? (s == 0 ? opt->wannier_u_up : opt->wannier_u_dn) : nullptr;
+            if (!U) continue;
+            const int N = c->nocc[s];
+            std::vector<double> Ut((size_t)N * N);
+            for (int v = 0; v < N; ++v) for (int n = 0; n < N; ++n) Ut[(size_t)n * N + v] = U[(size_t)v * N + n];
+            INIT_CUDA(cudaMalloc((void**)&c->d_U[s], sizeof(double) * N * N));
+            INIT_CUDA(cudaMalloc((void**)&c->d_Ut[s], sizeof(double) * N * N));
+            INIT_CUDA(cudaMemcpy(c->d_U[s], U, sizeof(double) * N * N, cudaMemcpyHostToDevice));
+            INIT_CUDA(cudaMemcpy(c->d_Ut[s], Ut.data(), sizeof(double) * N * N, cudaMemcpyHostToDevice));
+        }
+        // real-space orbitals: one buffer per spin, or one shared buffer refilled on demand when two do not fit comfortably
+        {
+            size_t fr = 0, tot = 0; cudaMemGetInfo(&fr, &tot);
+            const size_t both = sizeof(double) * (size_t)nr * ((size_t)c->nocc[0] + c->nocc[1]);
+            c->phi_shared = nspin == 2 && both > (size_t)(0.3 * (double)fr);
+            if (c->phi_shared) {
+                INIT_CUDA(cudaMalloc((void**)&c->d_phi[0], sizeof(double) * nr * std::max(c->nocc[0], c->nocc[1])));
+                c->d_phi[1] = c->d_phi[0];
+            } else for (int s = 0; s < nspin; ++s) INIT_CUDA(cudaMalloc((void**)&c->d_phi[s], sizeof(double) * nr * c->nocc[s]));
+        }
+        // rho0 and LDA f_xc (Eq. 8); spin-flip kernel of Eq. 26
         for (int a = 0; a < 3; ++a) INIT_CUDA(cudaMalloc((void**)&c->d_fxc[a], sizeof(double) * nr));
         {
             double *ru = nullptr, *rd = nullptr;
             INIT_CUDA(cudaMalloc((void**)&ru, sizeof(double) * nr));
-            INIT_CUDA(launch_rho0(c->d_phi[0], c->nocc[0], nr, ru, c->stream));
-            if (nspin == 2) { INIT_CUDA(cudaMalloc((void**)&rd, sizeof(double) * nr)); INIT_CUDA(launch_rho0(c->d_phi[1], c->nocc[1], nr, rd, c->stream)); }
+            if (nspin == 2) INIT_CUDA(cudaMalloc((void**)&rd, sizeof(double) * nr));
+            for (int s = nspin - 1; s >= 0; --s) {          // spin 0 last: a shared buffer then holds the spin the first apply starts with
+                c->phi_spin = -1;
+                int rc = compute_phi(c, s);
+                if (rc) { std::string m = c->err; cudaFree(ru); cudaFree(rd); return fail(rc, m); }
+                c->phi_spin = s;
+                INIT_CUDA(launch_rho0(c->d_phi[s], c->nocc[s], nr, s == 0 ? ru : rd, c->stream));
+            }
             INIT_CUDA(launch_lda_fxc(ru, nspin == 2 ? rd : ru, nr, c->rho_floor, c->d_fxc[0], c->d_fxc[1], c->d_fxc[2], c->stream));
+            if (c->sf_xc) {
+                INIT_CUDA(cudaMalloc((void**)&c->d_fsf, sizeof(double) * nr));
+                INIT_CUDA(launch_sf_kernel_table(ru, rd, nr, c->rho_floor, c->sf_cut, c->d_fsf, c->stream));
+            }
             INIT_CUDA(cudaStreamSynchronize(c->stream));
             cudaFree(ru); cudaFree(rd);
+        }
+        // near-sightedness truncation: explicit pair list, or overlap threshold on Eq. 32
+        for (int s = 0; s < nspin; ++s) {
+            const int* pl = opt ? (s == 0 ? opt->pair_list_up : opt->pair_list_dn) : nullptr;
+            const long np = opt ? (s == 0 ? opt->n_pairs_up : opt->n_pairs_dn) : 0;
+            const int N = c->nocc[s];
+            if (pl) {
+                c->mask[s].assign((size_t)N * N, 0);
+                for (long q = 0; q < np; ++q) {
+                    const int m = pl[2 * q], n = pl[2 * q + 1];
+                    if (m < 0 || n < 0 || m >= N || n >= N) return fail(TDDFT_EINVAL, "init: pair_list index out of range");
+                    c->mask[s][(size_t)m * N + n] = 1; c->mask[s][(size_t)n * N + m] = 1;
+                }
+            } else if (opt && opt->s_thr > 0) {
+                std::vector<double> S((size_t)N * N);
+                int rc = orbital_overlap(c, s, S.data());
+                if (rc) { std::string m = c->err; return fail(rc, m); }
+                c->mask[s].assign((size_t)N * N, 0);
+                for (size_t e = 0; e < S.size(); ++e) c->mask[s][e] = S[e] >= opt->s_thr ? 1 : 0;
+            }
+        }
+        if (opt && opt->ace) {
+            for (int s = 0; s < nspin; ++s) {
+                int rc = build_ace(c, s, s == 0 ? opt->psi_ace_up : opt->psi_ace_dn, s == 0 ? opt->n_ace_extra_up : opt->n_ace_extra_dn);
+                if (rc) { std::string m = c->err; return fail(rc, m); }
+            }
         }
 #undef INIT_CUDA
     } catch (const std::bad_alloc&) { return fail(TDDFT_ENOMEM, "init: host allocation failed"); }
@@ -567,6 +745,7 @@ int tddft_apply_liouville_host(tddft_ctx* c, const double* Xh, double* AXh, int 
     if (!c || !Xh || !AXh || nvec < 1 || mode < 0 || mode > 2) return TDDFT_EINVAL;
     const long L = vector_len(c, mode);
     if (L < 0) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    TD_CUDA(c, cudaSetDevice(c->device));
     const size_t bytes = sizeof(cplx) * (size_t)L * nvec;
     if (c->host_bytes < bytes) {      // staging buffers are kept between calls (allocation and release of GBs costs milliseconds)
         cudaFree(c->host_dx); cudaFree(c->host_dax); c->host_dx = c->host_dax = nullptr; c->host_bytes = 0;
@@ -625,7 +804,7 @@ int tddft_set_timing(tddft_ctx* c, int enabled) { if (!c) return TDDFT_EINVAL; c
 int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) {
     if (!c || !out) return TDDFT_EINVAL;
     *out = c->stats; out->fft_batch = c->fft_batch; out->fft_path = c->fused ? 0 : 1;
-    out->pair_batch = c->last_pair_batch; out->pair_tile = c->last_pair_tile;
+    out->pair_batch = c->last_pair_batch; out->pair_tile = c->last_pair_tile; out->k_chunk = c->last_kc; out->blocks_resident = c->last_resident;
     return TDDFT_OK;
 }
 
@@ -633,10 +812,13 @@ int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs
     if (!c || !pairs || !tau || n_pairs < 0 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
     for (long i = 0; i < 2 * n_pairs; ++i) if (pairs[i] < 0 || pairs[i] >= c->nocc[spin]) return set_err(c, TDDFT_EINVAL, "pair index out of range");
     if (n_pairs == 0) return TDDFT_OK;
+    TD_CUDA(c, cudaSetDevice(c->device));
+    TD_RC(ensure_phi(c, spin));
     int2* d = nullptr;
     TD_CUDA(c, cudaMalloc((void**)&d, sizeof(int2) * n_pairs));
     cudaError_t e = cudaMemcpyAsync(d, pairs, sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, c->stream);
-    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], d, nullptr, n_pairs, 2 * c->fft_batch, tau, 0) : set_err(c, TDDFT_ECUDA, "pair list copy failed");
+    int rc = (e == cudaSuccess) ? pair_potentials_dev(c, c->d_phi[spin], c->d_phi[spin], d, nullptr, n_pairs, 2 * c->fft_batch, tau, 0, n_pairs)
+                                : set_err(c, TDDFT_ECUDA, "pair list copy failed");
     cudaStreamSynchronize(c->stream);
     cudaFree(d);
     return rc;
@@ -644,6 +826,7 @@ int tddft_pair_potentials(tddft_ctx* c, int spin, const int* pairs, long n_pairs
 
 int tddft_project(tddft_ctx* c, int spin, double* Y, long nfun) {
     if (!c || !Y || nfun < 1 || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
+    TD_CUDA(c, cudaSetDevice(c->device));
     const size_t cap = project_scratch_doubles(c, c->nocc[spin], (int)nfun, (size_t)1 << 34);
     int rc = ensure_arena(c, sizeof(double) * cap);
     if (rc) return rc;
@@ -652,6 +835,7 @@ int tddft_project(tddft_ctx* c, int spin, double* Y, long nfun) {
 
 int tddft_gram(tddft_ctx* c, const double* V, const double* W, int m, long n_complex, double* G) {
     if (!c || !V || !W || !G || m < 1 || n_complex < 1) return TDDFT_EINVAL;
+    TD_CUDA(c, cudaSetDevice(c->device));
     const long K = 2 * n_complex;
     int splits = (int)std::max<long>(1, std::min<long>(1024, K / 8192));
     int rc = ensure_arena(c, sizeof(double) * (size_t)m * m * (splits + 1));
@@ -663,8 +847,15 @@ int tddft_gram(tddft_ctx* c, const double* V, const double* W, int m, long n_com
     return TDDFT_OK;
 }
 
+int tddft_orbital_overlap(tddft_ctx* c, int spin, double* S) {
+    if (!c || !S || spin < 0 || spin >= c->nspin) return TDDFT_EINVAL;
+    try { cudaSetDevice(c->device); return orbital_overlap(c, spin, S); }
+    catch (const std::bad_alloc&) { return set_err(c, TDDFT_ENOMEM, "overlap: host allocation failed"); }
+}
+
 int tddft_orbital_real_space(tddft_ctx* c, int spin, int v, double* out) {
     if (!c || !out || spin < 0 || spin >= c->nspin || v < 0 || v >= c->nocc[spin]) return TDDFT_EINVAL;
+    TD_RC(ensure_phi(c, spin));
     TD_CUDA(c, cudaMemcpyAsync(out, c->d_phi[spin] + (long)v * c->hp.nr, sizeof(double) * c->hp.nr, cudaMemcpyDeviceToDevice, c->stream));
     return TDDFT_OK;
 }

@@ -8,6 +8,10 @@
 
 namespace tddft {
 
+// Per-device caches of function attributes and occupancy (one process may hold contexts on several GPUs): index = device id.
+constexpr int kMaxDevices = 64;
+inline int current_device() { int d = 0; cudaGetDevice(&d); return (d >= 0 && d < kMaxDevices) ? d : 0; }
+
 // ---- FFT pass launchers (fft_inst.cu; one translation unit per size group) ---------------------------
 enum ZLoadKind { ZL_WORK = 0, ZL_PAIR = 1, ZL_PACK2 = 2 };
 enum ZStoreKind { ZS_WORK = 0, ZS_SPLIT2 = 1 };
@@ -23,6 +27,7 @@ struct ZArgs {
     cplx* work;            // [batch][nr] complex work grids (source for ZL_WORK, destination for ZS_WORK)
     // ZL_PAIR: packed grid b = phi[pairs[2b].x]*phi[pairs[2b].y] + i phi[pairs[2b+1].x]*phi[pairs[2b+1].y]
     const double* phi;     // [norb][nr]
+    const double* phi2;    // second operand array of the pair products, plain [nfun][nr]; null = phi (pairs of orbitals)
     const int2* pairs;     // device, npairs entries (already offset to this launch)
     int npairs;
     // ZL_PACK2: re = scale*(src0[2b] + src1[2b]), im = same for 2b+1 (src1 optional); nfun functions

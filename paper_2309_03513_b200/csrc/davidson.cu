@@ -7,7 +7,6 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <vector>
 #include "ctx.h"
 
@@ -147,6 +146,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     if (!evals || nroots < 1 || mode < 0 || mode > 2) return set_err(c, TDDFT_EINVAL, "davidson: bad argument");
     const long L = vector_len(c, mode);
     if (L < 0) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    TD_CUDA(c, cudaSetDevice(c->device));
     const long n2 = 2 * L, npwh = c->hp.npwh;
     cudaStream_t st = c->stream;
     const int max_sub = c->dav_max_subspace > 0 ? c->dav_max_subspace : 12 * nroots;
@@ -242,7 +242,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     if (m == 0) { cleanup(); return set_err(c, TDDFT_EINVAL, "davidson: start vectors vanish after projection"); }
 
     std::vector<double> h_theta(max_sub), h_res(nroots, 0.0), h_r2(nroots * nroots);
-    const bool trace = getenv("TDDFT_DAV_TRACE") != nullptr;     // one line per iteration on stderr
+    const bool trace = c->verbose != 0;      // one line per iteration on stderr
     int it = 0, status = TDDFT_ENOTCONVERGED, nr = 0;
     for (it = 1; it <= max_iter; ++it) {
         if (mw < m) {      // W = A V for the new columns

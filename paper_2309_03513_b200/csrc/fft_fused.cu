@@ -1,47 +1,36 @@
 // Instantiations and host dispatch of the fused FFT kernels (fft_fused.cuh) for the grid shapes of the BASELINE.json
 // configurations that fit the fast path; every other shape runs the general pass kernels (fft_steps.cuh).
-#include <cstdlib>
 #include <type_traits>
 #include "fft_fused.cuh"
 
 namespace tddft {
 
 // (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
-// columns: NY, NZ, threads and CTAs per SM, threads of the TMA-staged inverse kernel (one CTA per SM, one butterfly per
-// thread and stage; 0 = none)
-#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2, 648) X(48, 48, 96, 5, 0) X(24, 24, 96, 8, 0) X(18, 20, 96, 8, 0)
+#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8)
 #define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
 
-static int plane_variant() {          // tuning switch TDDFT_VAR: bit 0 persistent grid, bit 3 L2 prefetch of the next unit's orbital planes (off: they are shared with the units running now), bit 4 of its work-grid plane, bit 5 evict-first L2 policy on the work-grid / tau / a(r) streams, bit 6 TMA-staged inverse plane kernel
-    static int v = -1;
-    if (v < 0) { const char* e = getenv("TDDFT_VAR"); v = e ? atoi(e) : 49; }
-    return v;
-}
+// Launch policy, fixed after the round-1 measurements (profiles/r01g_summary.md, r01i_summary.md): persistent grids that walk
+// the units plane-major; L2 prefetch of the CTA's next work-grid plane (inverse kernels) but not of orbital planes (they are
+// shared with the units running now); evict-first L2 policy on the work-grid / tau / a(r) streams.
+constexpr int kStreamHint = 1;
 template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
 static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
     static_assert(Two<NY>::ok && Two<NZ>::ok, "fused plane kernel needs two-stage plans");
-    size_t smem = sizeof(cplx) * (size_t)NY * Two<NZ>::PITCH;
-    if (IsStaged<Load>::value) smem += sizeof(cplx) * (size_t)a.ncols + 16;      // stage + mbarrier
+    const size_t smem = sizeof(cplx) * (size_t)NY * Two<NZ>::PITCH;
     auto kern = plane_kernel<NY, NZ, NTHR, MINB, INV, DB1, DB2, Load, Store>;
-    static size_t attr_done = 0;
-    if (attr_done < smem) {
+    static int resident[kMaxDevices] = {0};                   // CTAs the device holds at once; 0 = attributes not set yet
+    const int dev = current_device();
+    if (!resident[dev]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done = smem;
+        int sms = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NTHR, smem);
+        resident[dev] = sms * (per_sm > 0 ? per_sm : 1);
     }
     const int nx = (int)(a.npencils / NY), nunits = nx * a.batch;
-    static int resident = 0;                                  // CTAs the device holds at once
-    static size_t resident_smem = 0;
-    if (!resident || resident_smem != smem) {
-        resident_smem = smem;
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NTHR, smem);
-        resident = sms * (per_sm > 0 ? per_sm : 1);
-    }
-    const int var = plane_variant();
-    const int grid = (var & 1) ? (nunits < resident ? nunits : resident) : nunits;
-    const int l2pf = std::is_same<Load, LoadWorkC>::value ? ((var & 16) ? 1 : 0) : ((var & 8) ? 1 : 0);
+    const int grid = nunits < resident[dev] ? nunits : resident[dev];
+    const int l2pf = std::is_same<Load, LoadWorkC>::value ? 1 : 0;
     kern<<<grid, NTHR, smem, s>>>(ld, st, nx, nunits, l2pf, a.tw2, a.tw);
     return cudaGetLastError();
 }
@@ -50,22 +39,16 @@ static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t 
     // double-buffered rounds (DB1 / DB2 of plane_kernel) measured slower on B200 (register pressure): both off
     return plane_launch2<NY, NZ, NTHR, MINB, INV, false, false>(ld, st, a, s);
 }
-template <int NY, int NZ, int NTHR, int MINB, int TSTAGED>
+template <int NY, int NZ, int NTHR, int MINB>
 static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
-    const int hint = (plane_variant() & 32) ? 1 : 0;
+    const int hint = kStreamHint;
     LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols, hint};
     StoreWorkC sw{a.work, a.wstride, a.cmap, a.ncols, hint};
     const BatchLayout lay{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr};
     if (!inverse) {
-        if (lkind == ZL_PAIR) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
+        if (lkind == ZL_PAIR) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.phi2 ? a.phi2 : a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
         if (lkind == ZL_PACK2) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPack2{a.src0, a.src1, a.nfun, lay, a.lscale}, sw, a, s);
         return cudaErrorInvalidValue;
-    }
-    if constexpr (TSTAGED > 0) {
-        // staged variant (TDDFT_VAR bit 6, opt-in) when the plane, the stage and the barrier fit one CTA's shared memory
-        const size_t need = sizeof(cplx) * ((size_t)NY * Two<NZ>::PITCH + (size_t)a.ncols) + 16;
-        if (skind == ZS_SPLIT2 && (plane_variant() & 64) && need <= 227 * 1024)
-            return plane_launch<NY, NZ, TSTAGED, 1, true>(LoadWorkT{a.work, a.wstride, a.cmap, a.ncols, hint}, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);
     }
     if (skind == ZS_SPLIT2) return plane_launch<NY, NZ, NTHR, MINB, true>(lw, StoreSplit2{a.dst, a.nfun, lay, a.sscale, hint, a.slots}, a, s);
     return cudaErrorInvalidValue;
@@ -75,24 +58,22 @@ template <int NX>
 static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     static_assert(Two<NX>::ok, "fused x pass needs a two-stage plan");
     constexpr size_t smem = XCfg<NX>::SMEM;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static int resident_d[kMaxDevices] = {0};
+    const int dev = current_device();
+    if (!resident_d[dev]) {
         cudaError_t e = cudaFuncSetAttribute(xpass_kernel<NX, SM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_CONV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        int sms = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_kernel<NX, SM_CONV>, XCfg<NX>::NTHR, smem);
+        resident_d[dev] = sms * (per_sm > 0 ? per_sm : 1);
     }
+    const int resident = resident_d[dev];
     // batch groups: enough CTAs for ~6 waves of the resident set, each CTA keeps its twiddles and Coulomb-table values
     // in registers while it walks over its grids
     const unsigned tiles = (unsigned)((a.inner + XW - 1) / XW);
-    static int resident = 0;
-    if (!resident) {
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_kernel<NX, SM_CONV>, XCfg<NX>::NTHR, smem);
-        resident = sms * (per_sm > 0 ? per_sm : 1);
-    }
     int gy = a.batch, best_gy = a.batch; double best = 0.0;
     for (gy = 1; gy <= a.batch; ++gy) {
         if ((long)tiles * gy < 3L * resident && gy < a.batch) continue;      // at least 3 waves (or one grid per CTA)
@@ -101,12 +82,11 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
         const double eff = (double)ctas / (double)(waves * resident) * (double)a.batch / (double)(per * gy);
         if (eff > best + 1e-9) { best = eff; best_gy = gy; }
     }
-    { static int force = -1; if (force < 0) { const char* e = getenv("TDDFT_XGY"); force = e ? atoi(e) : 0; } if (force > 0) best_gy = force < a.batch ? force : a.batch; }
     dim3 grid(tiles, (unsigned)best_gy);
     constexpr int NT = XCfg<NX>::NTHR;
-    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, (plane_variant() & 32) ? 1 : 0);
-    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, (plane_variant() & 32) ? 1 : 0);
-    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, (plane_variant() & 32) ? 1 : 0);
+    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
     return cudaGetLastError();
 }
 
@@ -115,13 +95,13 @@ bool fused_supported(const int* n) {
 #define X(N) if (n[0] == N) px = true;
     TD_FOR_EACH_XLEN(X)
 #undef X
-#define X(NY, NZ, T, B, TS) if (n[1] == NY && n[2] == NZ) pl = true;
+#define X(NY, NZ, T, B) if (n[1] == NY && n[2] == NZ) pl = true;
     TD_FOR_EACH_PLANE(X)
 #undef X
     return px && pl;
 }
 cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st) {
-#define X(NY, NZ, T, B, TS) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B, TS>(inverse, lkind, skind, a, st);
+#define X(NY, NZ, T, B) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B>(inverse, lkind, skind, a, st);
     TD_FOR_EACH_PLANE(X)
 #undef X
     return cudaErrorInvalidValue;

@@ -81,53 +81,10 @@ struct BStoreWorkC {
     cplx* g; const int* cmap; unsigned long long pol;
     __device__ __forceinline__ void operator()(int off, cplx v) const { const int c = __ldg(cmap + off); if (c >= 0) st_pol(g + c, v, pol); }
 };
-// TMA-staged variant of LoadWorkC: the compact plane of the CTA's next unit (one contiguous run of ncols complex numbers)
-// is pulled into a shared-memory stage by one bulk async copy (cp.async.bulk, completion on an mbarrier) while the CTA
-// transforms the current unit, so the first butterflies read shared memory and no warp waits on global loads.
-struct LoadWorkT { const cplx* work; long gstride; const int* cmap; int ncols; int hint; };
-struct BLoadWorkT {
-    const cplx* stage; const int* cmap;
-    typedef cplx Raw;
-    static constexpr int kModes = 1;
-    __device__ __forceinline__ int mode() const { return 0; }
-    template <int M> __device__ __forceinline__ Raw fetch(int off) const {
-        const int c = __ldg(cmap + off);
-        return c >= 0 ? stage[c] : make_double2(0.0, 0.0);
-    }
-    __device__ __forceinline__ Raw fetch_col(int c) const { return c >= 0 ? stage[c] : make_double2(0.0, 0.0); }
-    __device__ __forceinline__ cplx make(const Raw& r) const { return r; }
-    __device__ __forceinline__ void prefetch_l2(int, int, int) const {}
-};
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* smem, const void* gmem, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 template <class L> struct HasColMap { static constexpr bool value = false; };      // loads that go through the pruned column map
 template <> struct HasColMap<LoadWorkC> { static constexpr bool value = true; };
-template <> struct HasColMap<LoadWorkT> { static constexpr bool value = true; };
 template <class S> struct StoresColMap { static constexpr bool value = false; };  // stores that go through the pruned column map
 template <> struct StoresColMap<StoreWorkC> { static constexpr bool value = true; };
-template <class L> struct IsStaged { static constexpr bool value = false; };
-template <> struct IsStaged<LoadWorkT> { static constexpr bool value = true; };
 struct BLoadPair {
     const double *a0, *a1, *b0, *b1;   // re = a0*a1, im = imw*b0*b1 (imw = 0 for the odd last pair, which reuses a0, a1)
     double imw;
@@ -193,13 +150,12 @@ struct BStoreSplit2 {
     }
 };
 __device__ __forceinline__ BLoadWorkC bind(const LoadWorkC& l, int b, int x, long) { return BLoadWorkC{l.work + (long)b * l.gstride + (long)x * l.ncols, l.cmap, l.ncols, l2_policy(l.hint)}; }
-__device__ __forceinline__ BLoadWorkT bind(const LoadWorkT& l, int, int, long) { return BLoadWorkT{nullptr, l.cmap}; }
 __device__ __forceinline__ BStoreWorkC bind(const StoreWorkC& s, int b, int x, long) { return BStoreWorkC{s.work + (long)b * s.gstride + (long)x * s.ncols, s.cmap, l2_policy(s.hint)}; }
 __device__ __forceinline__ BLoadPair bind(const LoadPair& l, int b, int, long pbase) {
     const int2 p0 = l.pairs[2 * b];
-    BLoadPair r{l.phi + (long)p0.x * l.nr + pbase, l.phi + (long)p0.y * l.nr + pbase, nullptr, nullptr, 0.0};
+    BLoadPair r{l.phi + (long)p0.x * l.nr + pbase, l.phi2 + (long)p0.y * l.nr + pbase, nullptr, nullptr, 0.0};
     r.b0 = r.a0; r.b1 = r.a1;
-    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr + pbase; r.b1 = l.phi + (long)p1.y * l.nr + pbase; r.imw = 1.0; }
+    if (2 * b + 1 < l.npairs) { const int2 p1 = l.pairs[2 * b + 1]; r.b0 = l.phi + (long)p1.x * l.nr + pbase; r.b1 = l.phi2 + (long)p1.y * l.nr + pbase; r.imw = 1.0; }
     return r;
 }
 __device__ __forceinline__ BLoadPack2 bind(const LoadPack2& l, int b, int, long pbase) {
@@ -263,7 +219,6 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
     } else load_twiddles<R1y>(twy_g, tid % R2y, wy);
     typedef decltype(bind(ld, 0, 0, 0L)) BL;
     typedef typename BL::Raw Raw;
-    constexpr bool STAGED = IsStaged<Load>::value;
     const int nbatch = nunits / nx;
     constexpr int NR0 = (NZ * R1y + NTHR - 1) / NTHR;   // rounds of the first inverse stage
     int ccol[HasColMap<Load>::value ? NR0 : 1][R2y];
@@ -300,27 +255,10 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
             }
         }
     }
-    static_assert(!STAGED || INV, "only the inverse kernel reads staged work grids");
-    cplx* stage = sm + NY * PITCH;                      // STAGED: [ncols] compact plane, then the mbarrier
-    unsigned long long* mbar = nullptr;
-    unsigned parity = 0;
-    if constexpr (STAGED) {
-        mbar = (unsigned long long*)(stage + ld.ncols);
-        if (tid == 0) {
-            mbar_init(mbar, 1);
-            if ((int)blockIdx.x < nunits) {
-                const int x0 = blockIdx.x / nbatch, b0 = blockIdx.x - x0 * nbatch;
-                mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
-                bulk_g2s(stage, ld.work + (long)b0 * ld.gstride + (long)x0 * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
-            }
-        }
-        __syncthreads();
-    }
 
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int xpl = u / nbatch, b = u - xpl * nbatch;
         BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
-        if constexpr (STAGED) { L.stage = stage; mbar_wait(mbar, parity); parity ^= 1; }
         const auto S = bind(st, b, xpl, (long)xpl * NY * NZ);
         {   // operands of the unit this CTA takes next -> L2
             const int un = u + gridDim.x;
@@ -451,14 +389,6 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
                     for (int i = 0; i < R2y; ++i) col[i * PITCH] = x[i];
                 });
             __syncthreads();
-            if constexpr (STAGED) {     // the stage is consumed: start the copy of this CTA's next unit behind the remaining stages
-                const int un = u + gridDim.x;
-                if (tid == 0 && un < nunits) {
-                    const int xn = un / nbatch, bn = un - xn * nbatch;
-                    mbar_expect_tx(mbar, (unsigned)(ld.ncols * sizeof(cplx)));
-                    bulk_g2s(stage, ld.work + (long)bn * ld.gstride + (long)xn * ld.ncols, (unsigned)(ld.ncols * sizeof(cplx)), mbar);
-                }
-            }
             // y inverse stage R1y (conjugate twiddle before the butterfly), in place
             run_rounds<NZ * R2y, NTHR, DB2, RegBuf<cplx, R1y>>(tid,
                 [&](int t, RegBuf<cplx, R1y>& q) {

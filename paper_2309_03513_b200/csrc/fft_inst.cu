@@ -45,6 +45,4 @@ cudaError_t TD_CAT(launch_spass_g, TD_GROUP)(int n, int mode, const SArgs& a, cu
         default: *found = false; return cudaSuccess;
     }
 }
-cudaError_t TD_CAT(fft_set_attrs_g, TD_GROUP)() { return cudaSuccess; }
-
 }  // namespace tddft

@@ -14,15 +14,15 @@ struct LoadWork {
     const cplx* work; long nr;
     __device__ __forceinline__ cplx operator()(int b, long idx) const { return work[(long)b * nr + idx]; }
 };
-struct LoadPair {
-    const double* phi; const int2* pairs; int npairs; long nr;
+struct LoadPair {      // pair p = (x, y): density phi[x] * phi2[y] (both plain [function][nr]; K1d: phi2 = phi)
+    const double* phi; const double* phi2; const int2* pairs; int npairs; long nr;
     __device__ __forceinline__ cplx operator()(int b, long idx) const {
         const int2 p0 = pairs[2 * b];
-        double re = phi[(long)p0.x * nr + idx] * phi[(long)p0.y * nr + idx];
+        double re = phi[(long)p0.x * nr + idx] * phi2[(long)p0.y * nr + idx];
         double im = 0.0;
         if (2 * b + 1 < npairs) {
             const int2 p1 = pairs[2 * b + 1];
-            im = phi[(long)p1.x * nr + idx] * phi[(long)p1.y * nr + idx];
+            im = phi[(long)p1.x * nr + idx] * phi2[(long)p1.y * nr + idx];
         }
         return make_double2(re, im);
     }
@@ -151,7 +151,7 @@ cudaError_t zpass_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, c
     StoreWork sw{a.work, a.nr};
     if (!inverse) {
         // forward passes always store to the work grids
-        if (lkind == ZL_PAIR) return zpass_launch<N, false>(LoadPair{a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
+        if (lkind == ZL_PAIR) return zpass_launch<N, false>(LoadPair{a.phi, a.phi2 ? a.phi2 : a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
         if (lkind == ZL_PACK2) return zpass_launch<N, false>(LoadPack2{a.src0, a.src1, a.nfun, BatchLayout{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr}, a.lscale}, sw, a, s);
         return zpass_launch<N, false>(lw, sw, a, s);
     }

@@ -88,11 +88,12 @@ __global__ void splitk_reduce_kernel(const double* __restrict__ partial, int spl
 template <class CFG>
 static cudaError_t nt_pipe_launch(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
                                   int M, int N, long K, long kper, long wperiod, double cscale, int splits, double* partial, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    static bool attr_done[kMaxDevices] = {false};
+    const int dev = current_device();
+    if (!attr_done[dev]) {
         cudaError_t e = cudaFuncSetAttribute(gemm_nt_pipe_kernel<CFG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM_NT);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[dev] = true;
     }
     dim3 grid((unsigned)((N + CFG::BN - 1) / CFG::BN), (unsigned)((M + CFG::BM - 1) / CFG::BM), (unsigned)splits);
     gemm_nt_pipe_kernel<CFG><<<grid, CFG::NTHR, CFG::SMEM_NT, st>>>(A, lda, B, ldb, bgrp, bstride_grp, C, ldc, M, N, K, kper, wperiod, cscale, splits, partial);
@@ -174,11 +175,12 @@ cudaError_t launch_gemm_tn_acc(const double* At, long ldat, const double* B, lon
                                long cstride_grp, int M, long N, int K, double cscale, cudaStream_t st) {
     const bool aligned = (ldat % 2 == 0) && (ldb % 2 == 0) && (((size_t)At | (size_t)B) % 16 == 0);
     if (aligned && M >= 96 && N >= 96) {
-        static bool attr_done = false;
-        if (!attr_done) {
+        static bool attr_done[kMaxDevices] = {false};
+        const int dev = current_device();
+        if (!attr_done[dev]) {
             cudaError_t e = cudaFuncSetAttribute(gemm_tn_pipe_kernel<TnBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TnBig::SMEM_TN);
             if (e != cudaSuccess) return e;
-            attr_done = true;
+            attr_done[dev] = true;
         }
         dim3 grid((unsigned)((N + TnBig::BN - 1) / TnBig::BN), (unsigned)((M + TnBig::BM - 1) / TnBig::BM));
         gemm_tn_pipe_kernel<TnBig><<<grid, TnBig::NTHR, TnBig::SMEM_TN, st>>>(At, ldat, B, ldb, C, ldc, cgrp, cstride_grp, M, N, K, cscale);

@@ -1,5 +1,5 @@
 // Pointwise, scatter/gather, contraction and LDA kernels of the Liouville hot path (hand-written CUDA, sm_100a).
-#include <cstdlib>
+#include <algorithm>
 #include "kernels.h"
 
 namespace tddft {
@@ -40,11 +40,16 @@ __global__ void gather_unpack2_kernel(const cplx* __restrict__ work, long nr, co
     const long oa = (long)(lay.k0 + fa % lay.kc) * lay.vec_len + lay.block_off + (long)va * lay.npwh;
     const long ob = (long)(lay.k0 + fb % lay.kc) * lay.vec_len + lay.block_off + (long)vb * lay.npwh;
     const bool hb = fb < nfun;
-    const double ea = eig[va], eb = hb ? eig[vb] : 0.0;
+    const double ea = X ? eig[va] : 0.0, eb = (X && hb) ? eig[vb] : 0.0;
     const cplx* w = work + (long)b * nr;
     for (long g = blockIdx.x * (long)blockDim.x + threadIdx.x; g < lay.npwh; g += (long)gridDim.x * blockDim.x) {
         const cplx zp = w[idx_p[g]], zm = w[idx_m[g]];
         // c_A = (Z(G) + conj Z(-G))/2,  c_B = (Z(G) - conj Z(-G))/(2i)
+        if (!X) {      // plain transform to the sphere, no D term
+            AX[oa + g] = make_double2(0.5 * scale * (zp.x + zm.x), 0.5 * scale * (zp.y - zm.y));
+            if (hb) AX[ob + g] = make_double2(0.5 * scale * (zp.y + zm.y), -0.5 * scale * (zp.x - zm.x));
+            continue;
+        }
         const double k = kin[g];
         cplx xa = X[oa + g];
         AX[oa + g] = make_double2(fma(0.5 * scale, zp.x + zm.x, (k - ea) * xa.x), fma(0.5 * scale, zp.y - zm.y, (k - ea) * xa.y));
@@ -137,16 +142,7 @@ cudaError_t launch_out_init(const double* phi, const double* V, const double* vl
 // S5: out[(i0+i)*kc+k][r] -= alpha * sum_j tau_ij(r) a[(j0+j)*kc+k][r]   (Eq. 6).
 // Per grid point this is a (ti x tj)(tj x kc) product whose matrices differ at every r: a batch of N_r small GEMMs,
 // run on the FP64 tensor pipe (mma.sync.m8n8k4.f64).  All real-space batches (tau, a, out) use the chunked layout
-// [nr/32][function][32].  One CTA owns one chunk of 32 grid points, one block of 32 output rows and one direction;
-// its 16 warps take 2 grid points each (32 accumulators per lane).  The operands stream through shared memory in a
-// 4-stage cp.async ring (4 columns per stage: 32 KB of tau + 16 KB of a; every global read is a coalesced 256-byte
-// row; 6 copies of 16 bytes per thread per stage with incrementally updated pointers), rows padded to 272 bytes so
-// that the 16-byte fragment reads are bank-conflict free.  (Bulk async copies were tried: 192 copies of 256 bytes per
-// stage are TMA-issue bound, 2.7x slower.)
-// Off-diagonal tiles use tau twice (out[I] += tau a[J] and out[J] += tau^T a[I]).  The 8 CTAs of a chunk (4 row blocks
-// x 2 directions) are adjacent in launch order and sweep the 4x4 blocks of the tile on a skewed schedule -- direction 1,
-// row block b visits column block (b+t)&3 at step t, direction 2 visits (b-t)&3 -- so both users of a block of tau
-// touch it at about the same time and the second read is an L2 hit: tau crosses HBM about once.
+// [nr/32][function][32].
 __device__ __forceinline__ void dmma884k(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -157,204 +153,6 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-constexpr int CT_AROWS = 128;                      // tau rows per stage: 32 rows x 4 columns
-constexpr int CT_STAGES = 4;
-struct ColSweep {        // the column starts (multiples of 4) a unit visits: blocks of 32 in skewed order, empty blocks skipped
-    int t, cs, cend, wb, dir, ncols;
-    __device__ void settle() {
-        while (t < 4) {
-            const int cb = (dir == 0 ? (wb + t) : (wb - t + 4)) & 3;
-            if (cs < 0) cs = cb * 32;
-            cend = min(cb * 32 + 32, ncols);
-            if (cs < cend) return;
-            ++t; cs = -1;
-        }
-    }
-    __device__ void init(int dir_, int wb_, int ncols_) { dir = dir_; wb = wb_; ncols = ncols_; t = 0; cs = -1; settle(); }
-    __device__ bool valid() const { return t < 4; }
-    __device__ void next() { cs += 4; if (cs >= cend) { ++t; cs = -1; } settle(); }
-};
-// DUAL = true: off-diagonal tile, dense slots slot(i,j) = i*tj + j, units 0-3 = direction 1, 4-7 = direction 2.
-// DUAL = false: diagonal tile (ti == tj, same orbital block): one direction, tau stored for i <= j only, packed
-// row-major (the order build_tiles emits the pairs), read symmetrically.
-// WARPS warps of 2 grid points each: one CTA owns 2*WARPS points of a chunk (WARPS = 8: half a chunk, two CTAs per SM,
-// so one CTA's pipeline fill and write-back overlap the other's DMMA loop).  The accumulators start from -out/alpha
-// (loaded while the ring fills), so the write-back is store-only.
-template <int NK, bool DUAL, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS, 16 / WARPS)
-contract_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau, const int* __restrict__ slot,
-                const double* __restrict__ zeros, int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
-    extern __shared__ __align__(16) double sm[];
-    constexpr int PTS = 2 * WARPS;                         // grid points per CTA
-    constexpr int PARTS = CHUNK / PTS;                     // CTAs that share a chunk
-    constexpr int PITCH = PTS + 2;                         // padded row pitch (doubles): conflict-free 16-byte fragment reads
-    constexpr int BROWS = 4 * 8 * NK;                      // rows of a per stage: 4 columns x (8*NK) trial vectors
-    constexpr int ROWS = CT_AROWS + BROWS;
-    constexpr int STAGE = ROWS * PITCH;                    // doubles
-    constexpr int NCOPY = ROWS / 32;                       // 16-byte copies per thread per stage (32 rows per pass)
-    constexpr int NCOPY_A = CT_AROWS / 32;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const long cidx = blockIdx.x >> 3;
-    const long chunk = cidx / PARTS;
-    const int pt0 = (int)(cidx % PARTS) * PTS;             // first point of this CTA inside the chunk
-    const int unit = blockIdx.x & 7;
-    const int dir = DUAL ? (unit >> 2) : 0;
-    const int wb = DUAL ? (unit & 3) : (int)(blockIdx.y * 8 + unit);
-    const int nrows = dir == 0 ? ti : tj, ncols = dir == 0 ? tj : ti;
-    const int rowf0 = dir == 0 ? i0 : j0, colf0 = dir == 0 ? j0 : i0;
-    const int rb = wb * 32;
-    if (rb >= nrows) return;
-    const double* tau_c = tau + chunk * stot * CHUNK + pt0;
-    const double* a_c = a + chunk * ftot * CHUNK + pt0;
-    // this thread's copies: copy q moves piece (tid % WARPS) of stage row rc = q*32 + tid / WARPS
-    const int piece2 = (tid % WARPS) * 2;
-    const int rsub = tid / WARPS;                          // 0..31
-    const long a_colstride = (long)kc * CHUNK;             // next column of a
-    // out-of-range rows and columns are zero-filled with plain shared-memory stores
-    auto load_stage = [&](int buf, int cs) {
-        double* base = sm + buf * STAGE;
-#pragma unroll
-        for (int q = 0; q < NCOPY; ++q) {
-            const int rc = q * 32 + rsub;
-            const double* src = nullptr;
-            if (q < NCOPY_A) {
-                const int row = rb + (rc >> 2), col = cs + (rc & 3);
-                if (row < nrows && col < ncols) {
-                    long sl;
-                    if (DUAL) sl = dir == 0 ? (long)row * tj + col : (long)col * tj + row;
-                    else {   // diagonal tile: upper triangle packed row-major, slot(i,j) = i(2 tj - i + 1)/2 + (j - i), i <= j
-                        const int lo = min(row, col), hi = max(row, col);
-                        sl = (long)lo * (2 * tj - lo + 1) / 2 + (hi - lo);
-                    }
-                    src = tau_c + sl * CHUNK + piece2;
-                }
-            } else {
-                const int qq = rc - CT_AROWS;
-                const int k = qq >> 2, col = cs + (qq & 3);
-                if (col < ncols && k < kn) src = a_c + (long)(colf0 + col) * a_colstride + (long)k * CHUNK + piece2;
-            }
-            double* dst = base + rc * PITCH + piece2;
-            if (src) cp_async16(dst, src);
-            else *(double2*)dst = make_double2(0.0, 0.0);
-        }
-    };
-    ColSweep issue, use;
-    issue.init(dir, DUAL ? wb : 0, ncols);
-    use = issue;
-    const int lr = lane >> 2, lc = lane & 3;
-#pragma unroll
-    for (int st = 0; st < CT_STAGES - 1; ++st) {
-        if (issue.valid()) { load_stage(st, issue.cs); issue.next(); }
-        cp_async_commit();
-    }
-    // accumulators start from -out/alpha while the ring fills
-    double acc[4][NK][2][2];
-    double* out_c = out + chunk * ftot * CHUNK + pt0 + warp * 2;
-    const double minv = -1.0 / alpha;
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        const int i = rb + m * 8 + lr;
-#pragma unroll
-        for (int n = 0; n < NK; ++n)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int k = n * 8 + 2 * lc + h;
-                double2 x = make_double2(0.0, 0.0);
-                if (i < nrows && k < kn) x = *(const double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK);
-                acc[m][n][0][h] = x.x * minv; acc[m][n][1][h] = x.y * minv;
-            }
-    }
-    for (int step = 0; use.valid(); use.next(), ++step) {
-        const int buf = step % CT_STAGES;
-        cp_async_wait<CT_STAGES - 2>();
-        __syncthreads();                                     // stage `step` has landed for every thread; the previous buffer is free
-        if (issue.valid()) { load_stage((step + CT_STAGES - 1) % CT_STAGES, issue.cs); issue.next(); }
-        cp_async_commit();
-        const double* As = sm + buf * STAGE + warp * 2;
-        const double* Bs = As + CT_AROWS * PITCH;
-        double2 af[4], bf[NK];
-#pragma unroll
-        for (int m = 0; m < 4; ++m) af[m] = *(const double2*)(As + ((m * 8 + lr) * 4 + lc) * PITCH);
-#pragma unroll
-        for (int n = 0; n < NK; ++n) bf[n] = *(const double2*)(Bs + ((n * 8 + lr) * 4 + lc) * PITCH);
-#pragma unroll
-        for (int m = 0; m < 4; ++m)
-#pragma unroll
-            for (int n = 0; n < NK; ++n) {
-                dmma884k(acc[m][n][0][0], acc[m][n][0][1], af[m].x, bf[n].x);
-                dmma884k(acc[m][n][1][0], acc[m][n][1][1], af[m].y, bf[n].y);
-            }
-    }
-    cp_async_wait<0>();
-    const double malpha = -alpha;
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        const int i = rb + m * 8 + lr;
-        if (i >= nrows) continue;
-#pragma unroll
-        for (int n = 0; n < NK; ++n)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int k = n * 8 + 2 * lc + h;
-                if (k >= kn) continue;
-                *(double2*)(out_c + ((long)(rowf0 + i) * kc + k) * CHUNK) = make_double2(malpha * acc[m][n][0][h], malpha * acc[m][n][1][h]);
-            }
-    }
-}
-
-static int contract_warps() {      // points per CTA = 2 * warps: 8 (two CTAs per SM, default) or 16
-    static int w = 0;
-    if (!w) { const char* e = getenv("TDDFT_CT_WARPS"); w = (e && atoi(e) == 16) ? 16 : 8; }
-    return w;
-}
-template <int NK, bool DUAL, int WARPS>
-static cudaError_t contract_launch2(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
-                                    int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    const size_t smem = sizeof(double) * CT_STAGES * (CT_AROWS + 4 * 8 * NK) * (2 * WARPS + 2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(contract_kernel<NK, DUAL, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    grid.x *= CHUNK / (2 * WARPS);
-    contract_kernel<NK, DUAL, WARPS><<<grid, 32 * WARPS, smem, st>>>(out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
-    return cudaGetLastError();
-}
-template <int NK, bool DUAL>
-static cudaError_t contract_launch(dim3 grid, double* out, const double* a, const double* tau, const int* slot, const double* zeros,
-                                   int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    if (contract_warps() == 16) return contract_launch2<NK, DUAL, 16>(grid, out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-    return contract_launch2<NK, DUAL, 8>(grid, out, a, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-}
-cudaError_t launch_contract_single(double* out, const double* a, const double* tau, const int* slot, const double* zeros, int i0, int ti,
-                                   int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st) {
-    const long nchunks = (nr + CHUNK - 1) / CHUNK;
-    dim3 grid((unsigned)(nchunks * 8), (unsigned)((ti + 255) / 256));
-    for (int kb = 0; kb < kc; kb += 16) {
-        const int kn = kc - kb < 16 ? kc - kb : 16;
-        double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
-        cudaError_t e = kn > 8 ? contract_launch<2, false>(grid, o, ap, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                               : contract_launch<1, false>(grid, o, ap, tau, slot, zeros, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
-}
-cudaError_t launch_contract_dual(double* out, const double* a, const double* tau, const double* zeros, int i0, int ti, int j0, int tj,
-                                 int kc, long ftot, long nr, double alpha, cudaStream_t st) {
-    if (ti > 128 || tj > 128) return cudaErrorInvalidValue;
-    const long nchunks = (nr + CHUNK - 1) / CHUNK;
-    dim3 grid((unsigned)(nchunks * 8));
-    for (int kb = 0; kb < kc; kb += 16) {
-        const int kn = kc - kb < 16 ? kc - kb : 16;
-        double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
-        cudaError_t e = kn > 8 ? contract_launch<2, true>(grid, o, ap, tau, nullptr, zeros, i0, ti, j0, tj, kc, kn, ftot, (long)ti * tj, alpha, st)
-                               : contract_launch<1, true>(grid, o, ap, tau, nullptr, zeros, i0, ti, j0, tj, kc, kn, ftot, (long)ti * tj, alpha, st);
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
-}
 
 // ------------------------------------------------------------------------------------------------------
 // S5, register-resident tiles.  One warp owns ONE grid point and keeps the whole row block of the tile in registers:
@@ -571,11 +369,12 @@ template <int NK, bool DIAG, class SH>
 static cudaError_t contract_full_launch(long nchunks, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj,
                                         int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
     constexpr size_t smem = FullCfg<NK, SH>::SMEM;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static bool attr_done[kMaxDevices] = {false};
+    const int dev = current_device();
+    if (!attr_done[dev]) {
         cudaError_t e = cudaFuncSetAttribute(contract_full_kernel<NK, DIAG, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done[dev] = true;
     }
     contract_full_kernel<NK, DIAG, SH><<<(unsigned)(nchunks * (CHUNK / FT_P)), 32 * FT_P, smem, st>>>(out, a, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
     return cudaGetLastError();
@@ -602,6 +401,131 @@ cudaError_t launch_contract_full(bool diag, double* out, const double* a, const 
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// V[kk][r] = f[r] * d[kk][r]: the spin-flip K1e potential f^SF * drho^SF (Eq. 24)
+__global__ void scale_potential_kernel(const double* __restrict__ f, const double* __restrict__ d, long nr, double* __restrict__ V) {
+    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (r >= nr) return;
+    const long o = (long)blockIdx.y * nr + r;
+    V[o] = f[r] * d[o];
+}
+cudaError_t launch_scale_potential(const double* f, const double* d, int kc, long nr, double* V, cudaStream_t st) {
+    dim3 grid((unsigned)((nr + 255) / 256), (unsigned)kc);
+    scale_potential_kernel<<<grid, 256, 0, st>>>(f, d, nr, V);
+    return cudaGetLastError();
+}
+
+// D term alone (Eq. 3 with the kinetic model H): AX[f][g] = (kin[g] - eig[v]) X[f][g] for the functions of one spin block
+__global__ void d_term_kernel(const cplx* __restrict__ X, cplx* __restrict__ AX, FunLayout lay, int nfun, const double* __restrict__ kin,
+                              const double* __restrict__ eig) {
+    const int f = blockIdx.y;
+    const int v = f / lay.kc;
+    const long o = (long)(lay.k0 + f % lay.kc) * lay.vec_len + lay.block_off + (long)v * lay.npwh;
+    const double e = eig[v];
+    for (long g = blockIdx.x * (long)blockDim.x + threadIdx.x; g < lay.npwh; g += (long)gridDim.x * blockDim.x) {
+        const cplx x = X[o + g];
+        const double d = kin[g] - e;
+        AX[o + g] = make_double2(d * x.x, d * x.y);
+    }
+}
+cudaError_t launch_d_term(const cplx* X, cplx* AX, FunLayout lay, int nfun, const double* kin, const double* eig, cudaStream_t st) {
+    dim3 grid((unsigned)std::min<long>(64, (lay.npwh + 255) / 256), (unsigned)nfun);
+    d_term_kernel<<<grid, 256, 0, st>>>(X, AX, lay, nfun, kin, eig);
+    return cudaGetLastError();
+}
+
+// out[f0 + (t - t_first)*fstep][r] += scale * sum_{j < nj} M[j][r] * tau[j*nt + t][r],  t_first <= t < t_first + t_count
+// (the sum over bands of Eq. 7 / Eq. 28: PAPER.md:95-96, :201-204).  M plain [j][nr]; tau chunked [nr/32][nj*nt][32];
+// out chunked [nr/32][ftot][32].
+template <int KT>
+__global__ void pattern_reduce_kernel(const double* __restrict__ M, const double* __restrict__ tau, int nj, int nt, int t0, int tend, long nr,
+                                      double* __restrict__ out, long ftot, long f0, long fstep, double scale) {
+    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (r >= nr) return;
+    double acc[KT];
+#pragma unroll
+    for (int q = 0; q < KT; ++q) acc[q] = 0.0;
+    const double* tc = tau + (r >> 5) * ((long)nj * nt * CHUNK) + (r & (CHUNK - 1));
+    for (int j = 0; j < nj; ++j) {
+        const double m = M[(long)j * nr + r];
+        const double* tj = tc + ((long)j * nt + t0) * CHUNK;
+#pragma unroll
+        for (int q = 0; q < KT; ++q) if (t0 + q < tend) acc[q] = fma(m, tj[q * CHUNK], acc[q]);
+    }
+    double* oc = out + (r >> 5) * (ftot * CHUNK) + (r & (CHUNK - 1));
+#pragma unroll
+    for (int q = 0; q < KT; ++q) if (t0 + q < tend) { double* o = oc + (f0 + (long)q * fstep) * CHUNK; *o = fma(scale, acc[q], *o); }
+}
+cudaError_t launch_pattern_reduce(const double* M, const double* tau, int nj, int nt, int t_first, int t_count, long nr, double* out, long ftot,
+                                  long f0, long fstep, double scale, cudaStream_t st) {
+    const unsigned nb = (unsigned)((nr + 127) / 128);
+    for (int t0 = t_first; t0 < t_first + t_count; t0 += 4)
+        pattern_reduce_kernel<4><<<nb, 128, 0, st>>>(M, tau, nj, nt, t0, t_first + t_count, nr, out, ftot, f0 + (long)(t0 - t_first) * fstep, fstep, scale);
+    return cudaGetLastError();
+}
+
+// sq[v][r] = phi[v][r]^2 (the densities of Eq. 32)
+__global__ void square_kernel(const double* __restrict__ phi, long n, double* __restrict__ sq) {
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) { const double p = phi[i]; sq[i] = p * p; }
+}
+cudaError_t launch_square(const double* phi, long n, double* sq, cudaStream_t st) {
+    square_kernel<<<(unsigned)std::min<long>(65535, (n + 255) / 256), 256, 0, st>>>(phi, n, sq);
+    return cudaGetLastError();
+}
+
+__global__ void symmetrize_kernel(double* __restrict__ H, int m, double scale) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m * m) return;
+    const int r = i / m, c = i % m;
+    if (r < c) { const double v = 0.5 * scale * (H[r * m + c] + H[c * m + r]); H[r * m + c] = v; H[c * m + r] = v; }
+    else if (r == c) H[i] *= scale;
+}
+cudaError_t launch_symmetrize(double* H, int m, double scale, cudaStream_t st) {
+    symmetrize_kernel<<<(m * m + 255) / 256, 256, 0, st>>>(H, m, scale);
+    return cudaGetLastError();
+}
+
+// Cholesky A = L L^T of a small symmetric positive definite matrix and the inverse of L, one CTA, in global memory
+// (ACE: M = -L L^T, xi = W L^-T, Eq. 30).  A [n][n] row-major is overwritten by L (lower triangle);
+// Linv [n][n] receives L^-1 (lower triangular, zeros above).  status[0] = 0 or the 1-based index of a non-positive pivot.
+__global__ void __launch_bounds__(1024) chol_inv_kernel(double* __restrict__ A, double* __restrict__ Linv, int n, int* __restrict__ status) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    __shared__ double piv;
+    __shared__ int bad;
+    if (tid == 0) bad = 0;
+    __syncthreads();
+    for (int k = 0; k < n; ++k) {
+        if (tid == 0) { const double d = A[(long)k * n + k]; if (!(d > 0.0)) { bad = k + 1; piv = 1.0; } else piv = sqrt(d); }
+        __syncthreads();
+        if (bad) break;
+        const double p = piv;
+        for (int i = k + tid; i < n; i += nt) A[(long)i * n + k] = (i == k) ? p : A[(long)i * n + k] / p;
+        __syncthreads();
+        // trailing update of the lower triangle: A[i][j] -= L[i][k] L[j][k], k < j <= i
+        const int m = n - k - 1;
+        for (long e = tid; e < (long)m * m; e += nt) {
+            const int i = k + 1 + (int)(e / m), j = k + 1 + (int)(e % m);
+            if (j <= i) A[(long)i * n + j] -= A[(long)i * n + k] * A[(long)j * n + k];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) status[0] = bad;
+    if (bad) return;
+    // columns of L^-1 by forward substitution, one column per thread: L x = e_c
+    for (int c = tid; c < n; c += nt) {
+        for (int i = 0; i < n; ++i) {
+            if (i < c) { Linv[(long)i * n + c] = 0.0; continue; }
+            double sacc = (i == c) ? 1.0 : 0.0;
+            for (int j = c; j < i; ++j) sacc -= A[(long)i * n + j] * Linv[(long)j * n + c];
+            Linv[(long)i * n + c] = sacc / A[(long)i * n + i];
+        }
+    }
+}
+cudaError_t launch_chol_inv(double* A, double* Linv, int n, int* status, cudaStream_t st) {
+    chol_inv_kernel<<<1, 1024, 0, st>>>(A, Linv, n, status);
+    return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -670,6 +594,35 @@ __global__ void lda_fxc_kernel(const double* __restrict__ rho_up, const double* 
 cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double* fuu, double* fud,
                            double* fdd, cudaStream_t st) {
     lda_fxc_kernel<<<(unsigned)((nr + 255) / 256), 256, 0, st>>>(rho_up, rho_dn, nr, rho_floor, fuu, fud, fdd);
+    return cudaGetLastError();
+}
+
+// Spin-flip xc kernel of Eq. 26: f^SF = (V_xc,up - V_xc,dn) / (rho_up - rho_dn), zero where
+// |rho_up - rho_dn| < cut.  V_xc by hand: v_x,s = -(6 rho_s/pi)^(1/3);
+// v_c,s = eps - (rs/3) eps_rs + (s - zeta) eps_zeta, so v_c,up - v_c,dn = 2 eps_zeta = 2 f'(zeta) (eps_P - eps_U).
+// The potentials are evaluated at densities clamped from below at rho_floor (reading A5).
+__global__ void sf_kernel_table(const double* __restrict__ rho_up, const double* __restrict__ rho_dn, long nr, double rho_floor,
+                                double cut, double* __restrict__ fsf) {
+    const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (r >= nr) return;
+    const double d = rho_up[r] - rho_dn[r];
+    if (!(fabs(d) >= cut)) { fsf[r] = 0.0; return; }
+    const double ru = fmax(rho_up[r], rho_floor), rd = fmax(rho_dn[r], rho_floor);
+    const double rho = ru + rd, zeta = (ru - rd) / rho;
+    const double rs = cbrt(3.0 / (4.0 * M_PI * rho));
+    const PZ U = {-0.1423, 1.0529, 0.3334, 0.0311, -0.048, 0.0020, -0.0116};
+    const PZ P = {-0.0843, 1.3981, 0.2611, 0.01555, -0.0269, 0.0007, -0.0048};
+    double eu, eu1, eu2, ep, ep1, ep2;
+    pz_eps(U, rs, eu, eu1, eu2);
+    pz_eps(P, rs, ep, ep1, ep2);
+    const double c0 = 2.0 * cbrt(2.0) - 2.0;
+    const double fz1 = (4.0 / 3.0) * (cbrt(1.0 + zeta) - cbrt(1.0 - zeta)) / c0;
+    const double dvx = -cbrt(6.0 / M_PI) * (cbrt(ru) - cbrt(rd));
+    fsf[r] = (dvx + 2.0 * fz1 * (ep - eu)) / d;
+}
+cudaError_t launch_sf_kernel_table(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double cut, double* fsf,
+                                   cudaStream_t st) {
+    sf_kernel_table<<<(unsigned)((nr + 255) / 256), 256, 0, st>>>(rho_up, rho_dn, nr, rho_floor, cut, fsf);
     return cudaGetLastError();
 }
 

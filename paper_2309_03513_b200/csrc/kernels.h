@@ -14,7 +14,7 @@ struct FunLayout {
 // S1: sphere -> zeroed complex work grids, two functions per grid (re/im), functions f0 .. f0+2*batch-1 (< nfun)
 cudaError_t launch_scatter_pack2(const cplx* X, FunLayout lay, int f0, int nfun, int batch, const int* idx_p, const int* idx_m,
                                  cplx* work, long nr, cudaStream_t st);
-// S6+S7: work grids -> sphere with scale, plus (kin[g] - eig[v]) * x(g)  (Eq. 3)
+// S6+S7: work grids -> sphere with scale, plus (kin[g] - eig[v]) * x(g)  (Eq. 3); X = null: no D term
 cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, const int* idx_m, int f0, int nfun, int batch,
                                   double scale, const cplx* X, cplx* AX, FunLayout lay, const double* kin, const double* eig,
                                   cudaStream_t st);
@@ -30,18 +30,23 @@ cudaError_t launch_out_init(const double* phi, const double* V, const double* vl
                             double* out, cudaStream_t st);
 // S5 (Eq. 6) on batches in the chunked layout [nr/32][function][32] (common.h); ftot = functions in
 // a/out (nocc*kc), stot = slots in the tau tile.
-// single: out[(i0+i)*kc+k] -= alpha sum_{j<tj} tau[slot[i*tj+j]] a[(j0+j)*kc+k]    (diagonal tiles; slot table on device)
-// dual:   that with slot(i,j) = i*tj+j AND out[(j0+j)*kc+k] -= alpha sum_i tau[i*tj+j] a[(i0+i)*kc+k]   (off-diagonal tiles)
-cudaError_t launch_contract_single(double* out, const double* a, const double* tau, const int* slot, const double* zeros, int i0, int ti,
-                                   int j0, int tj, int kc, long ftot, long stot, long nr, double alpha, cudaStream_t st);
-cudaError_t launch_contract_dual(double* out, const double* a, const double* tau, const double* zeros, int i0, int ti, int j0, int tj,
-                                 int kc, long ftot, long nr, double alpha, cudaStream_t st);   // zeros: 256 B of device zeros
-// S5, register-resident variant: one launch does a whole tile with up to contract_full_max_tile() rows (any number of
+// Register-resident tiles: one launch does a whole tile with up to contract_full_max_tile() rows (any number of
 // columns); diag: ti == tj, same orbital block, tau packed upper-triangular (one direction, symmetric reads); else dense
 // slots i*tj + j and both directions.  stot = slots in the tau tile.
 int contract_full_max_tile();
 cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
                                  long ftot, long stot, long nr, double alpha, cudaStream_t st);
+// spin-flip K1e potential V[kk][r] = f[r] * d[kk][r] (Eq. 24); D term alone AX = (kin - eig_v) X (Eq. 3)
+cudaError_t launch_scale_potential(const double* f, const double* d, int kc, long nr, double* V, cudaStream_t st);
+cudaError_t launch_d_term(const cplx* X, cplx* AX, FunLayout lay, int nfun, const double* kin, const double* eig, cudaStream_t st);
+// out[f0 + (t - t_first)*fstep] += scale * sum_j M[j] * tau[j*nt + t], t_first <= t < t_first + t_count (Eq. 7 / Eq. 28 band sums)
+cudaError_t launch_pattern_reduce(const double* M, const double* tau, int nj, int nt, int t_first, int t_count, long nr, double* out, long ftot,
+                                  long f0, long fstep, double scale, cudaStream_t st);
+cudaError_t launch_square(const double* phi, long n, double* sq, cudaStream_t st);
+cudaError_t launch_symmetrize(double* H, int m, double scale, cudaStream_t st);   // H <- scale (H + H^T)/2
+cudaError_t launch_chol_inv(double* A, double* Linv, int n, int* status, cudaStream_t st);
+cudaError_t launch_sf_kernel_table(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double cut, double* fsf,
+                                   cudaStream_t st);
 // S0: rho[r] = sum_v phi[v][r]^2 ; LDA kernel f_xc (Eq. 8; reading A5)
 cudaError_t launch_rho0(const double* phi, int nocc, long nr, double* rho, cudaStream_t st);
 cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, double rho_floor, double* fuu, double* fud,

@@ -10,7 +10,7 @@ class Case:
     """Holds the same inputs for both sides.  The CUDA side is created lazily (needs a GPU)."""
 
     def __init__(self, lattice, grid, ecut, nspin, nocc, alpha, seed, envelope=True, ortho="lowdin",
-                 vloc=False, use_hartree_fxc=True, fft_backend="radix", oracle=True, **gpu_opts):
+                 vloc=False, use_hartree_fxc=True, fft_backend="radix", oracle=True, oracle_opts=None, psi=None, **gpu_opts):
         self.lattice = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
         self.grid = tuple(grid); self.ecut = ecut; self.nspin = nspin; self.nocc = tuple(nocc); self.alpha = alpha
         self.use_hartree_fxc = use_hartree_fxc
@@ -18,7 +18,7 @@ class Case:
         self.miller, self.g2 = olat.enumerate_half_sphere(self.lattice, ecut)
         self.npwh = len(self.miller)
         self.rng = np.random.Generator(np.random.PCG64(seed))
-        self.psi = [inputs.orbitals(self.rng, nocc[s], self.g2, ecut, envelope, ortho) for s in range(nspin)]
+        self.psi = psi if psi is not None else [inputs.orbitals(self.rng, nocc[s], self.g2, ecut, envelope, ortho) for s in range(nspin)]
         self.eig = [inputs.eigenvalues(self.rng, nocc[s]) for s in range(nspin)]
         self.vloc = None
         if vloc:
@@ -27,7 +27,7 @@ class Case:
         self.oracle = None
         if oracle:
             self.oracle = olv.Problem(self.lattice, self.grid, ecut, nspin, self.psi, self.eig, alpha,
-                                      use_hartree_fxc=use_hartree_fxc, vloc=self.vloc, fft_backend=fft_backend)
+                                      use_hartree_fxc=use_hartree_fxc, vloc=self.vloc, fft_backend=fft_backend, **(oracle_opts or {}))
         self._ctx = None
 
     @classmethod

@@ -88,12 +88,46 @@ def test_apply_config2_sampled_columns():
     _invariants(case, X, got, 0)
 
 
+# Columns (k, spin block, v) sampled at config 3.  The tau tiles are 108 orbitals wide (432 = 4 x 108; spin down 430 = 3 x 108 + 106,
+# a ragged last tile): the v values hit every row-tile class 0-107, 108-215, 216-323, 324-431 of spin up, both ends of the ragged
+# last block of spin down (v = 324..429), the first and last orbital, and k covers both halves of the 16-vector DMMA batch
+# (k = 0, 7, 8, 15).  One column per mode is computed with the oracle's own radix FFT instead of the library transform.
+CFG3_COLUMNS = {
+    0: [(0, 0, 0), (0, 0, 431), (7, 0, 107), (7, 0, 108), (8, 0, 215), (8, 0, 216), (15, 0, 323), (15, 0, 324),
+        (0, 1, 0), (7, 1, 150), (8, 1, 324), (15, 1, 429)],
+    1: [(0, 0, 0), (0, 0, 431), (7, 0, 107), (7, 0, 200), (8, 0, 216), (8, 0, 323), (15, 0, 324), (15, 0, 108)],
+}
+CFG3_RADIX_COLUMN = {0: (8, 1, 324), 1: (7, 0, 200)}
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 def test_apply_config3_sampled_columns(mode):
     # BASELINE.json configs[2], the bench workload: 72^3, 432/430 orbitals, 16 trial vectors, both modes
-    case = Case.from_config(3, fft_backend="numpy")   # library FFT as the oracle's transform step (pinned equal to the radix FFT)
+    case = Case.from_config(3, fft_backend="numpy")   # library FFT as the oracle's transform step (pinned equal to the radix FFT at 72^3)
     X = case.trial(16, mode)
     got = case.gpu_apply(X, mode)
-    samples = [(3, 0, 431), (3, 1, 17)] if mode == 0 else [(11, 0, 200)]
-    assert _sampled_columns(case, X, got, mode, samples) < TOL
+    assert _sampled_columns(case, X, got, mode, CFG3_COLUMNS[mode]) < TOL
     _invariants(case, X, got, mode)
+    # one column through the oracle's own radix transform
+    o = case.oracle
+    k, s, v = CFG3_RADIX_COLUMN[mode]
+    ctx = o.prepare(X[k], mode)
+    o.fft_backend = "radix"
+    ref = o.column(ctx, s, v)
+    o.fft_backend = "numpy"
+    a = (o.nocc[0] * o.npwh if (mode == 0 and s == 1) else 0) + v * o.npwh
+    assert rel_fro(got.reshape(16, -1)[k, a:a + o.npwh], ref) < TOL
+
+
+@pytest.mark.parametrize("grid,lattice,ecut,nocc,nvec", [
+    # the three-stage plans of the general pass kernels, never reached by the smaller grids: 96 = 6*4*4, 100 = 10*10, 108 = 3*6*6,
+    # 128 = 8*4*4 (fft_core.cuh); the shapes of BASELINE.json configs[3] (hexagonal) and [4] and of the 60 Ry workload
+    ((96, 96, 100), [[12.0, 0, 0], [-6.0, 12.0 * 0.8660254037844386, 0], [0, 0, 8.0]], 5.0, (4, 3), 2),
+    ((108, 108, 108), [[9.0, 0, 0], [0, 9.0, 0], [0, 0, 9.0]], 8.0, (4, 3), 2),
+    ((128, 128, 128), [[9.0, 0, 0], [0, 9.0, 0], [0, 0, 9.0]], 8.0, (3, 2), 1),
+])
+def test_apply_large_fft_plans(grid, lattice, ecut, nocc, nvec):
+    case = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid))      # oracle with its own radix FFT
+    for mode in (0, 1):
+        X = case.trial(nvec, mode)
+        assert rel_fro(case.gpu_apply(X, mode), case.oracle.apply(X, mode)) < TOL

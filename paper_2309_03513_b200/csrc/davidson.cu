@@ -117,19 +117,102 @@ __global__ void symmetrize_kernel(double* __restrict__ H, int m) {
     const int r = i / m, c = i % m;
     if (r < c) { const double v = 0.5 * (H[r * m + c] + H[c * m + r]); H[r * m + c] = v; H[c * m + r] = v; }
 }
-// counter-based normal numbers (splitmix64 + Box-Muller) for the library's own start vectors
-__device__ __forceinline__ unsigned long long splitmix(unsigned long long x) {
-    x += 0x9E3779B97F4A7C15ull; x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull; x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
-    return x ^ (x >> 31);
+// ---- projector-aware correction (reading A11b of DESIGN.md) ----------------------------------------------------------------
+// For every function v of a spin block and Ritz value theta: solve P_c (T - lambda_v) P_c t = r on range(P_c), lambda_v = eps_v + theta:
+//   t = M^-1 (r - Phi c),  c = S^-1 Phi^T M^-1 r,  S = Phi^T M^-1 Phi,  M = diag(|G|^2/2 - lambda_v) with |M| floored at 1e-2 (sign kept).
+constexpr double kDenFloor = 1e-2;
+__device__ __forceinline__ double pc_den(double kin, double lam) {
+    double d = kin - lam;
+    if (fabs(d) < kDenFloor) d = d < 0 ? -kDenFloor : kDenFloor;
+    return d;
 }
-__global__ void random_start_kernel(cplx* __restrict__ x, long L, long npwh, unsigned long long seed, double amp, long unit_elem) {
-    for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < L; e += (long)gridDim.x * blockDim.x) {
-        const unsigned long long a = splitmix(seed + 2ull * (unsigned long long)e), b = splitmix(seed + 2ull * (unsigned long long)e + 1ull);
-        const double u1 = ((double)(a >> 11) + 0.5) * (1.0 / 9007199254740992.0), u2 = ((double)(b >> 11) + 0.5) * (1.0 / 9007199254740992.0);
-        const double rad = amp * sqrt(-2.0 * log(u1));
-        double s, c; sincospi(2.0 * u2, &s, &c);
-        x[e] = make_double2(rad * c + (e == unit_elem ? 1.0 : 0.0), (e % npwh == 0) ? 0.0 : rad * s);
+__global__ void pc_lambda_kernel(const double* __restrict__ eig, const double* __restrict__ theta, int root, int n, double* __restrict__ lam) {
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v < n) lam[v] = eig[v] + theta[root];
+}
+// weighted != 0: out[v][k] = gamma_k in[v][k] / d_v(k) (gamma: the Gamma inner-product weights 2, 1 for Re c(0), 0 for Im c(0));
+// weighted == 0: out[v][k] = in[v][k] / d_v(k)
+__global__ void pc_divide_kernel(const double* __restrict__ in, double* __restrict__ out, long k2, const double* __restrict__ kin,
+                                 const double* __restrict__ lam, int weighted) {
+    const int v = blockIdx.y;
+    const double l = lam[v];
+    const double* src = in + (long)v * k2; double* dst = out + (long)v * k2;
+    for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < k2; k += (long)gridDim.x * blockDim.x) {
+        const double d = pc_den(kin[k >> 1], l);
+        double w = 1.0 / d;
+        if (weighted) w = (k >= 2) ? 2.0 / d : (k == 0 ? 1.0 / d : 0.0);
+        dst[k] = src[k] * w;
     }
+}
+__global__ void fill_kernel(double* __restrict__ x, int n, double v) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) x[i] = v;
+}
+// w[row][k] = kin[k/2] x[row][k]: the kinetic operator on half-sphere functions stored as 2 npwh reals
+__global__ void kin_mul_kernel(const double* __restrict__ x, double* __restrict__ w, long k2, const double* __restrict__ kin) {
+    const double* src = x + (long)blockIdx.y * k2; double* dst = w + (long)blockIdx.y * k2;
+    for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < k2; k += (long)gridDim.x * blockDim.x) dst[k] = kin[k >> 1] * src[k];
+}
+__global__ void unit_kernel(double* __restrict__ x, long k2, long idx) {
+    for (long k = blockIdx.x * (long)blockDim.x + threadIdx.x; k < k2; k += (long)gridDim.x * blockDim.x) x[k] = k == idx ? 1.0 : 0.0;
+}
+// One CTA solves one dense system S x = b by Gaussian elimination with partial pivoting (S is symmetric but indefinite: M has both
+// signs), right-hand side carried along in shared memory.  S [nsys][n][n] is destroyed.  The solution leaves negated and
+// transposed: CT[u][v0 + sys] = -x[u], the operand of the GEMM  t = r - sum_u c_u phi_u.
+__global__ void __launch_bounds__(512) lu_solve_kernel(double* __restrict__ Sall, const double* __restrict__ Ball, double* __restrict__ CT,
+                                                      int ldct, int n, int v0) {
+    extern __shared__ double sh[];
+    double* prow = sh; double* lcol = sh + n; double* x = sh + 2 * n;
+    __shared__ double redv[16]; __shared__ int redi[16]; __shared__ int piv;
+    double* A = Sall + (size_t)blockIdx.x * n * n;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+    for (int i = tid; i < n; i += blockDim.x) x[i] = Ball[(size_t)blockIdx.x * n + i];
+    __syncthreads();
+    for (int k = 0; k < n; ++k) {
+        double bv = -1.0; int bi = k;
+        for (int i = k + tid; i < n; i += blockDim.x) { const double a = fabs(A[(size_t)i * n + k]); if (a > bv) { bv = a; bi = i; } }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_down_sync(0xffffffffu, bv, o); const int oi = __shfl_down_sync(0xffffffffu, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) { redv[warp] = bv; redi[warp] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            double b = redv[0]; int p = redi[0];
+            for (int w = 1; w < nw; ++w) if (redv[w] > b || (redv[w] == b && redi[w] < p)) { b = redv[w]; p = redi[w]; }
+            piv = p;
+        }
+        __syncthreads();
+        const int p = piv;
+        if (p != k) {
+            for (int j = k + tid; j < n; j += blockDim.x) { const double a = A[(size_t)k * n + j]; A[(size_t)k * n + j] = A[(size_t)p * n + j]; A[(size_t)p * n + j] = a; }
+            if (tid == 0) { const double a = x[k]; x[k] = x[p]; x[p] = a; }
+            __syncthreads();
+        }
+        for (int j = k + tid; j < n; j += blockDim.x) prow[j] = A[(size_t)k * n + j];
+        __syncthreads();
+        double pv = prow[k];
+        if (fabs(pv) < 1e-300) pv = 1e-300;          // exactly singular S (lambda on the spectrum of P_c T P_c): regularised
+        for (int i = k + 1 + tid; i < n; i += blockDim.x) lcol[i] = A[(size_t)i * n + k] / pv;
+        __syncthreads();
+        const double xk = x[k];
+        for (int i = k + 1 + warp; i < n; i += nw) {
+            const double l = lcol[i];
+            double* row = A + (size_t)i * n;
+            for (int j = k + 1 + lane; j < n; j += 32) row[j] = fma(-l, prow[j], row[j]);
+            if (lane == 0) x[i] = fma(-l, xk, x[i]);
+        }
+        __syncthreads();
+    }
+    for (int k = n - 1; k >= 0; --k) {
+        if (tid == 0) { double pv = A[(size_t)k * n + k]; if (fabs(pv) < 1e-300) pv = 1e-300; x[k] /= pv; }
+        __syncthreads();
+        const double xk = x[k];
+        for (int i = tid; i < k; i += blockDim.x) x[i] = fma(-A[(size_t)i * n + k], xk, x[i]);
+        __syncthreads();
+    }
+    for (int i = tid; i < n; i += blockDim.x) CT[(size_t)i * ldct + v0 + blockIdx.x] = -x[i];
 }
 
 }  // namespace
@@ -166,7 +249,8 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     double *V = nullptr, *W = nullptr, *XR = nullptr, *T = nullptr, *small = nullptr, *Oproj = nullptr;
     const int splits = (int)std::max<long>(1, std::min<long>(256, n2 / 65536));
     const size_t small_n = (size_t)max_sub * max_sub * (3 + splits) + 4 * max_sub + 64;
-    auto cleanup = [&]() { cudaFree(V); cudaFree(W); cudaFree(XR); cudaFree(T); cudaFree(small); cudaFree(Oproj); cudaGetLastError(); };
+    double *pcS = nullptr, *pcRS = nullptr, *pcB = nullptr, *pcLam = nullptr, *fbuf_owner = nullptr, *Ufun = nullptr;
+    auto cleanup = [&]() { cudaFree(fbuf_owner); cudaFree(Ufun); cudaFree(V); cudaFree(W); cudaFree(XR); cudaFree(T); cudaFree(small); cudaFree(Oproj); cudaFree(pcS); cudaFree(pcRS); cudaFree(pcB); cudaFree(pcLam); cudaGetLastError(); };
 #define DV_TRY(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { cleanup(); return set_err(c, e_ == cudaErrorMemoryAllocation ? TDDFT_ENOMEM : TDDFT_ECUDA, std::string("davidson: " #call ": ") + cudaGetErrorString(e_)); } } while (0)
 #define DV_RC(expr) do { int rc_ = (expr); if (rc_) { cleanup(); return rc_; } } while (0)
     DV_TRY(cudaMalloc((void**)&V, sizeof(double) * n2 * max_sub));
@@ -174,7 +258,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     DV_TRY(cudaMalloc((void**)&XR, sizeof(double) * n2 * 3 * nroots));     // X (Ritz), R (residual / W-combination), WY for restarts
     DV_TRY(cudaMalloc((void**)&T, sizeof(double) * n2));
     DV_TRY(cudaMalloc((void**)&small, sizeof(double) * small_n));
-    const size_t oproj_cap = project_scratch_doubles(c, maxocc, maxocc, (size_t)1 << 34);
+    const size_t oproj_cap = project_scratch_doubles(c, maxocc, std::max(maxocc, 16), (size_t)1 << 34);
     DV_TRY(cudaMalloc((void**)&Oproj, sizeof(double) * oproj_cap));
     double* X = XR; double* R = XR + n2 * nroots; double* WY = XR + 2 * n2 * nroots;
     double* H = small; double* Hwork = H + (size_t)max_sub * max_sub; double* Y = Hwork + (size_t)max_sub * max_sub;
@@ -216,24 +300,161 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
         return TDDFT_OK;
     };
 
+    // projector-aware correction (reading A11b): rows t_v with P_c (T_kin - lam_v) P_c t_v = r_v for n functions of target spin tgt
+    const bool pc_aware = c->dav_precond == 0;
+    constexpr int PF = 4;                     // conduction functions per spin of the start-vector phase (reading A11c)
+    constexpr int FMAX = 8 * PF;
+    double* pcCT = nullptr;
+    int pc_chunk = 0;
+    {
+        int maxn = PF, maxt = 0;
+        for (auto& b : blocks) { maxn = std::max(maxn, c->nocc[b.src]); maxt = std::max(maxt, c->nocc[b.tgt]); }
+        const size_t per = sizeof(double) * (size_t)maxt * maxt;
+        pc_chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)maxn, ((size_t)2 << 30) / per));
+        DV_TRY(cudaMalloc((void**)&pcS, std::max(per * pc_chunk, sizeof(double) * 12 * (size_t)maxn * maxt)));   // also the k-split scratch of the rhs GEMM
+        DV_TRY(cudaMalloc((void**)&pcRS, sizeof(double) * (size_t)maxn * 2 * npwh));
+        DV_TRY(cudaMalloc((void**)&pcB, sizeof(double) * (size_t)maxn * maxt * 2));
+        DV_TRY(cudaMalloc((void**)&pcLam, sizeof(double) * maxn));
+        pcCT = pcB + (size_t)maxn * maxt;
+        cudaFuncSetAttribute(lu_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 3 * maxt));
+    }
+    auto solve_rows = [&](const double* rblk, double* tblk, int n, int tgt) -> int {      // shifts lam_v in pcLam[0..n)
+        const long k2 = 2 * npwh;
+        const int nt = c->nocc[tgt];
+        pc_divide_kernel<<<dim3(64, n), 256, 0, st>>>(rblk, pcRS, k2, c->d_kin, pcLam, 1);
+        TD_CUDA(c, cudaGetLastError());
+        // B[v][u] = <phi_u| M_v^-1 |r_v>
+        TD_CUDA(c, launch_gemm_nt(pcRS, k2, c->psi[tgt], k2, nt, 0, pcB, nt, n, nt, k2, 0, 1.0, 12, pcS, st));    // pcS doubles as the k-split scratch
+        for (int v0 = 0; v0 < n; v0 += pc_chunk) {
+            const int nv = std::min(pc_chunk, n - v0);
+            TD_CUDA(c, launch_gram_shift(c->psi[tgt], k2, nt, k2, c->d_kin, pcLam + v0, nv, kDenFloor, pcS, st));
+            lu_solve_kernel<<<nv, 512, sizeof(double) * 3 * nt, st>>>(pcS, pcB + (size_t)v0 * nt, pcCT, n, nt, v0);
+            TD_CUDA(c, cudaGetLastError());
+            launches += 2;
+        }
+        // t_v = M_v^-1 (r_v - sum_u c_v[u] phi_u)
+        if (tblk != rblk) TD_CUDA(c, cudaMemcpyAsync(tblk, rblk, sizeof(double) * (size_t)n * k2, cudaMemcpyDeviceToDevice, st));
+        TD_CUDA(c, launch_gemm_tn_acc(pcCT, n, c->psi[tgt], k2, tblk, k2, n, 0, n, k2, nt, 1.0, st));
+        pc_divide_kernel<<<dim3(64, n), 256, 0, st>>>(tblk, tblk, k2, c->d_kin, pcLam, 0);
+        TD_CUDA(c, cudaGetLastError());
+        launches += 5;
+        return TDDFT_OK;
+    };
+    auto precond_projector = [&](int root) -> int {      // T <- correction of root `root`, lam_v = eps_v + theta_root
+        for (auto& b : blocks) {
+            const int n = c->nocc[b.src];
+            pc_lambda_kernel<<<(n + 127) / 128, 128, 0, st>>>(c->d_eig[b.src], theta, root, n, pcLam);
+            int rc = solve_rows(R + (long)root * n2 + 2 * b.off, T + 2 * b.off, n, b.tgt); if (rc) return rc;
+        }
+        return TDDFT_OK;
+    };
+
+    // Start-vector phase (reading A11c of DESIGN.md): the PF lowest eigenfunctions u_m (eigenvalues mu_m) of P_c T P_c of one target
+    // spin, by a block Davidson in the space of single functions whose correction is the exact inverse at a fixed shift below the
+    // spectrum, t = (P_c (T - sigma) P_c)^-1 r with sigma = -0.05 Ha < 0 <= T (a positive definite solve: robust from any start).
+    // The eigenvectors of D alone (Eq. 3) are u_m (x) e_v with eigenvalue mu_m - eps_v; the lowest of them start the solver.
+    double*& fbuf = fbuf_owner;
+    auto conduction_functions = [&](int tgt, double* Uout, double* mu_host) -> int {
+        const long k2 = 2 * npwh;
+        const int fsplits = (int)std::max<long>(1, std::min<long>(64, k2 / 4096));
+        if (!fbuf) TD_CUDA(c, cudaMalloc((void**)&fbuf, sizeof(double) * ((size_t)(2 * FMAX + 3 * PF) * k2 + (size_t)FMAX * FMAX * (3 + fsplits) + 4 * FMAX + 64)));
+        double* FV = fbuf; double* FW = FV + (size_t)FMAX * k2; double* FX = FW + (size_t)FMAX * k2; double* FR = FX + (size_t)PF * k2;
+        double* FT = FR + (size_t)PF * k2; double* fH = FT + (size_t)PF * k2; double* fHw = fH + FMAX * FMAX; double* fY = fHw + FMAX * FMAX;
+        double* fpart = fY + FMAX * FMAX; double* ftheta = fpart + (size_t)FMAX * FMAX * fsplits; double* fcoef = ftheta + FMAX; double* fnrm = fcoef + 2 * FMAX;
+        const unsigned fb = (unsigned)std::min<long>(1024, (k2 + 255) / 256);
+        const size_t ocap = oproj_cap;
+        int fm = 0, fw = 0;
+        auto fproject = [&](double* x, int rows) { return project_rows(c, tgt, x, rows, rows, 0, Oproj, ocap); };
+        auto fgs_append = [&](double* t) -> int {      // two Gram-Schmidt passes against FV[0..fm), P_c, normalise, append
+            for (int pass = 0; pass < 2 && fm > 0; ++pass) {
+                TD_CUDA(c, launch_gemm_nt(FV, k2, t, k2, 1, 0, fcoef, 1, fm, 1, k2, k2, 2.0, fsplits, fpart, st));
+                TD_CUDA(c, launch_gemm_tn_acc(fcoef, 1, FV, k2, t, k2, 1, 0, 1, k2, fm, -1.0, st));
+            }
+            int rc = fproject(t, 1); if (rc) return rc;
+            TD_CUDA(c, launch_gemm_nt(t, k2, t, k2, 1, 0, fnrm, 1, 1, 1, k2, k2, 2.0, fsplits, fpart, st));
+            double q = 0; TD_CUDA(c, cudaMemcpyAsync(&q, fnrm, sizeof(double), cudaMemcpyDeviceToHost, st)); TD_CUDA(c, cudaStreamSynchronize(st));
+            if (q > 1e-20) { scale_kernel<<<fb, 256, 0, st>>>(t, k2, fnrm, FV + (size_t)fm * k2); TD_CUDA(c, cudaGetLastError()); ++fm; }
+            return TDDFT_OK;
+        };
+        for (int i = 0; i < PF && i + 1 < k2; ++i) {      // unit vectors on the lowest kinetic energies (real coordinates 0, 2, 3, 4, ...)
+            unit_kernel<<<fb, 256, 0, st>>>(FT, k2, i == 0 ? 0 : i + 1);
+            int rc = fproject(FT, 1); if (rc) return rc;
+            rc = fgs_append(FT); if (rc) return rc;
+        }
+        if (fm == 0) return set_err(c, TDDFT_EINVAL, "davidson: no conduction function found");
+        std::vector<double> hth(FMAX), hr2(PF * PF);
+        int np = 0;
+        for (int fit = 0; fit < 80; ++fit) {
+            if (fw < fm) {      // W = P_c T V on the new rows
+                kin_mul_kernel<<<dim3(fb, fm - fw), 256, 0, st>>>(FV + (size_t)fw * k2, FW + (size_t)fw * k2, k2, c->d_kin);
+                int rc = fproject(FW + (size_t)fw * k2, fm - fw); if (rc) return rc;
+                fw = fm;
+            }
+            TD_CUDA(c, launch_gemm_nt(FV, k2, FW, k2, fm, 0, fH, fm, fm, fm, k2, k2, 2.0, fsplits, fpart, st));
+            symmetrize_kernel<<<(fm * fm + 255) / 256, 256, 0, st>>>(fH, fm);
+            TD_CUDA(c, cudaMemcpyAsync(fHw, fH, sizeof(double) * fm * fm, cudaMemcpyDeviceToDevice, st));
+            { const int mp = (fm + 1) & ~1; jacobi_eigh_kernel<<<1, 512, sizeof(double) * mp + sizeof(int) * mp, st>>>(fHw, fH, fm, ftheta, fY); }
+            np = std::min(PF, fm);
+            TD_CUDA(c, cudaMemsetAsync(FX, 0, sizeof(double) * k2 * np, st));
+            TD_CUDA(c, cudaMemsetAsync(FR, 0, sizeof(double) * k2 * np, st));
+            TD_CUDA(c, launch_gemm_tn_acc(fY, fm, FV, k2, FX, k2, np, 0, np, k2, fm, 1.0, st));
+            TD_CUDA(c, launch_gemm_tn_acc(fY, fm, FW, k2, FR, k2, np, 0, np, k2, fm, 1.0, st));
+            residual_kernel<<<dim3(fb, np), 256, 0, st>>>(FR, FX, k2, ftheta);
+            TD_CUDA(c, launch_gemm_nt(FR, k2, FR, k2, np, 0, fHw, np, np, np, k2, k2, 2.0, fsplits, fpart, st));
+            TD_CUDA(c, cudaMemcpyAsync(hth.data(), ftheta, sizeof(double) * fm, cudaMemcpyDeviceToHost, st));
+            TD_CUDA(c, cudaMemcpyAsync(hr2.data(), fHw, sizeof(double) * np * np, cudaMemcpyDeviceToHost, st));
+            TD_CUDA(c, cudaStreamSynchronize(st));
+            bool all = np == PF || np == fm;
+            int nnew = 0;
+            for (int i = 0; i < np; ++i) if (std::sqrt(std::max(hr2[(size_t)i * np + i], 0.0)) > 1e-7) { all = false; ++nnew; }
+            if (c->verbose) { fprintf(stderr, "davidson start phase spin %d it %d m %d mu", tgt, fit, fm); for (int i = 0; i < np; ++i) fprintf(stderr, " %.6e (%.1e)", hth[i], std::sqrt(std::max(hr2[(size_t)i * np + i], 0.0))); fprintf(stderr, "\n"); }
+            if (all) break;
+            if (fm + nnew > FMAX) {      // restart from the Ritz functions
+                TD_CUDA(c, cudaMemsetAsync(FT, 0, sizeof(double) * k2 * np, st));
+                TD_CUDA(c, launch_gemm_tn_acc(fY, fm, FW, k2, FT, k2, np, 0, np, k2, fm, 1.0, st));
+                TD_CUDA(c, cudaMemcpyAsync(FV, FX, sizeof(double) * k2 * np, cudaMemcpyDeviceToDevice, st));
+                TD_CUDA(c, cudaMemcpyAsync(FW, FT, sizeof(double) * k2 * np, cudaMemcpyDeviceToDevice, st));
+                fm = np; fw = np;
+            }
+            fill_kernel<<<1, 64, 0, st>>>(pcLam, np, -0.05);
+            int rc = solve_rows(FR, FT, np, tgt); if (rc) return rc;
+            const int fm0 = fm;
+            for (int i = 0; i < np; ++i) {
+                if (std::sqrt(std::max(hr2[(size_t)i * np + i], 0.0)) <= 1e-7) continue;
+                rc = fproject(FT + (size_t)i * k2, 1); if (rc) return rc;
+                rc = fgs_append(FT + (size_t)i * k2); if (rc) return rc;
+            }
+            if (fm == fm0) break;
+        }
+        TD_CUDA(c, cudaMemcpyAsync(Uout, FX, sizeof(double) * k2 * np, cudaMemcpyDeviceToDevice, st));
+        TD_CUDA(c, cudaStreamSynchronize(st));
+        for (int i = 0; i < PF; ++i) mu_host[i] = i < np ? hth[i] : 1e300;
+        return TDDFT_OK;
+    };
+
     // ---- start vectors -------------------------------------------------------------------------------
     int m = 0, mw = 0;
-    std::vector<long> guess;
-    if (!(c->dav_x0 && c->dav_nx0 > 0)) {     // host index logic only: the nstart smallest diagonal elements, ties by position
-        std::vector<std::pair<double, long>> cand;
-        for (auto& b : blocks)
-            for (int v = 0; v < c->nocc[b.src]; ++v)
-                for (long g = 0; g < std::min<long>(npwh, nstart); ++g)
-                    cand.push_back({0.5 * c->hp.g2[g] - c->eig_h[b.src][v], b.off + (long)v * npwh + g});
-        std::sort(cand.begin(), cand.end());
-        for (int i = 0; i < nstart; ++i) guess.push_back(cand[std::min<size_t>(i, cand.size() - 1)].second);
+    struct Cand { double e; long off; int tgt, fun; };
+    std::vector<Cand> cand;
+    if (!(c->dav_x0 && c->dav_nx0 > 0)) {
+        // lowest eigenvectors of D (reading A11c): u_m (x) e_v over the blocks, ordered by mu_m - eps_v (host index logic only)
+        const long k2 = 2 * npwh;
+        DV_TRY(cudaMalloc((void**)&Ufun, sizeof(double) * 2 * PF * k2));
+        double mu[2][PF]; bool have[2] = {false, false};
+        for (auto& b : blocks) {
+            if (!have[b.tgt]) { DV_RC(conduction_functions(b.tgt, Ufun + (size_t)b.tgt * PF * k2, mu[b.tgt])); have[b.tgt] = true; }
+            for (int f = 0; f < PF; ++f)
+                for (int v = 0; v < c->nocc[b.src]; ++v)
+                    if (mu[b.tgt][f] < 1e299) cand.push_back({mu[b.tgt][f] - c->eig_h[b.src][v], b.off + (long)v * npwh, b.tgt, f});
+        }
+        std::sort(cand.begin(), cand.end(), [](const Cand& x, const Cand& y) { return x.e < y.e || (x.e == y.e && x.off < y.off); });
     }
     for (int i = 0; i < nstart; ++i) {
         if (c->dav_x0 && c->dav_nx0 > 0) DV_TRY(cudaMemcpyAsync(T, c->dav_x0 + (long)i * n2, sizeof(double) * n2, cudaMemcpyDeviceToDevice, st));
-        else {   // unit vector on the i-th smallest diagonal element |G|^2/2 - eps_v plus seeded noise of 2-norm ~1e-3 (reading A11):
-                 // the amplitude per component scales with 1/sqrt(2L), or the noise would swamp the unit vector at L ~ 10^7
-            random_start_kernel<<<eb, 256, 0, st>>>((cplx*)T, L, npwh, c->seed * 0x100000001B3ull + 0x51ED27ull + (unsigned long long)i * (unsigned long long)(2 * L + 2), 1e-3 / sqrt(2.0 * (double)L), guess[i]);
-            DV_TRY(cudaGetLastError()); ++launches;
+        else {
+            if (i >= (int)cand.size()) break;
+            DV_TRY(cudaMemsetAsync(T, 0, sizeof(double) * n2, st));
+            DV_TRY(cudaMemcpyAsync(T + 2 * cand[i].off, Ufun + ((size_t)cand[i].tgt * PF + cand[i].fun) * 2 * npwh, sizeof(double) * 2 * npwh, cudaMemcpyDeviceToDevice, st));
         }
         DV_RC(project_vec(T));
         double nr_ = 0; DV_RC(gs2(T, m, &nr_));
@@ -294,10 +515,12 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
             m = nr; mw = nr;
         }
         const int m_before = m;
-        for (int i = 0; i < nr; ++i) {
+        const int max_new = c->dav_block > 0 ? c->dav_block : nroots;
+        for (int i = 0, added = 0; i < nr && added < max_new; ++i) {
             if (h_res[i] <= tol) continue;
-            precondition_kernel<<<eb, 256, 0, st>>>((const cplx*)(R + (long)i * n2), (cplx*)T, L, npwh, pb, c->d_kin, theta, i);
-            DV_TRY(cudaGetLastError()); ++launches;
+            ++added;
+            if (pc_aware) DV_RC(precond_projector(i));
+            else { precondition_kernel<<<eb, 256, 0, st>>>((const cplx*)(R + (long)i * n2), (cplx*)T, L, npwh, pb, c->d_kin, theta, i); DV_TRY(cudaGetLastError()); ++launches; }
             DV_RC(project_vec(T));
             double n0 = 0, n1 = 0;
             { double q = 0; DV_RC(norm2_to_host(T, &q)); n0 = std::sqrt(std::max(q, 0.0)); }

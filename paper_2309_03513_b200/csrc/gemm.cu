@@ -131,6 +131,34 @@ cudaError_t launch_gemm_nt(const double* A, long lda, const double* B, long ldb,
     return cudaGetLastError();
 }
 
+cudaError_t launch_gram_shift(const double* Phi, long lda, int M, long K, const double* kin, const double* lam, int nb, double dfloor,
+                              double* S, cudaStream_t st) {
+    if (lda % 2 != 0 || ((size_t)Phi) % 16 != 0) return cudaErrorInvalidValue;
+    dim3 grid;
+    if (M >= 96) {
+        static bool attr_done[kMaxDevices] = {false};
+        const int dev = current_device();
+        if (!attr_done[dev]) {
+            cudaError_t e = cudaFuncSetAttribute(gram_shift_kernel<NtBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NtBig::SMEM_NT);
+            if (e != cudaSuccess) return e;
+            attr_done[dev] = true;
+        }
+        grid = dim3((unsigned)((M + NtBig::BN - 1) / NtBig::BN), (unsigned)((M + NtBig::BM - 1) / NtBig::BM), (unsigned)nb);
+        gram_shift_kernel<NtBig><<<grid, NtBig::NTHR, NtBig::SMEM_NT, st>>>(Phi, lda, M, K, kin, lam, dfloor, S);
+    } else {
+        static bool attr_done[kMaxDevices] = {false};
+        const int dev = current_device();
+        if (!attr_done[dev]) {
+            cudaError_t e = cudaFuncSetAttribute(gram_shift_kernel<NtSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NtSmall::SMEM_NT);
+            if (e != cudaSuccess) return e;
+            attr_done[dev] = true;
+        }
+        grid = dim3((unsigned)((M + NtSmall::BN - 1) / NtSmall::BN), (unsigned)((M + NtSmall::BM - 1) / NtSmall::BM), (unsigned)nb);
+        gram_shift_kernel<NtSmall><<<grid, NtSmall::NTHR, NtSmall::SMEM_NT, st>>>(Phi, lda, M, K, kin, lam, dfloor, S);
+    }
+    return cudaGetLastError();
+}
+
 __global__ void __launch_bounds__(128) gemm_tn_acc_kernel(const double* __restrict__ At, long ldat, const double* __restrict__ B, long ldb,
                                                           double* __restrict__ C, long ldc, int cgrp, long cstride_grp, int M, long N,
                                                           int K, double cscale) {

@@ -216,4 +216,101 @@ gemm_tn_pipe_kernel(const double* __restrict__ At, long ldat, const double* __re
     }
 }
 
+// Shifted, weighted Gram matrices of the projector-aware Davidson correction (reading A11b of DESIGN.md):
+//   S_b[u][u'] = sum_k Phi[u][k] Phi[u'][k] w_b[k],   w_b[k] = gamma_k / d,  d = kin[k/2] - lam[b] with |d| floored at dfloor (sign kept),
+// gamma_k = 2 (1 for Re c(G=0), 0 for Im c(G=0)): the Gamma inner product of <phi_u| (T - lambda)^-1 |phi_u'>.
+// Phi [M][K] K-contiguous (K = 2 npwh reals); blockIdx.z = b; S [nb][M][M].  Same pipeline as gemm_nt_pipe_kernel, the weight is
+// applied to the B fragments in registers.
+template <class CFG>
+__global__ void __launch_bounds__(CFG::NTHR, 1)
+gram_shift_kernel(const double* __restrict__ A, long lda, int M, long K, const double* __restrict__ kin, const double* __restrict__ lam,
+                  double dfloor, double* __restrict__ S) {
+    constexpr int BM = CFG::BM, BN = CFG::BN, LDK = CFG::LDK, ST = CFG::STAGES, NTHR = CFG::NTHR, FM = CFG::FM, FN = CFG::FN;
+    extern __shared__ __align__(16) double gsm[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm0 = (warp / CFG::WARPS_N) * CFG::WM, wn0 = (warp % CFG::WARPS_N) * CFG::WN;
+    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    const double lambda = lam[blockIdx.z];
+    const int KT = (int)((K + GK - 1) / GK);
+    constexpr int CHUNKS = (BM + BN) * (GK / 2);
+    constexpr int NQ = (CHUNKS + NTHR - 1) / NTHR;
+    const double* src[NQ]; int soff[NQ]; int kc2[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int ch = tid + q * NTHR;
+        const int row = ch / (GK / 2), kc = (ch % (GK / 2)) * 2;
+        src[q] = nullptr; soff[q] = row * LDK + kc; kc2[q] = kc;
+        if (ch < CHUNKS) {
+            const int r = row < BM ? m0 + row : n0 + row - BM;
+            if (r < M) src[q] = A + (long)r * lda + kc;
+        } else soff[q] = -1;
+    }
+    auto load_stage = [&](int buf, int kt) {
+        double* base = gsm + (size_t)buf * (BM + BN) * LDK;
+        const long krem = K - (long)kt * GK;
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            if (soff[q] < 0) continue;
+            long left = krem - kc2[q];
+            int bytes = (src[q] && left > 0) ? (left >= 2 ? 16 : 8) : 0;
+            cp16z(base + soff[q], bytes ? (const void*)(src[q] + (long)kt * GK) : (const void*)A, bytes);
+        }
+    };
+    double acc[FM][FN][2];
+#pragma unroll
+    for (int i = 0; i < FM; ++i)
+#pragma unroll
+        for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+    for (int s = 0; s < ST - 1; ++s) { if (s < KT) load_stage(s, s); cp_commit(); }
+    const int lr = lane >> 2, lc = lane & 3;
+    for (int kt = 0; kt < KT; ++kt) {
+        // this lane's weights of the stage: k = kt*GK + k0 + lc
+        double w[GK / 4];
+#pragma unroll
+        for (int q = 0; q < GK / 4; ++q) {
+            const long k = (long)kt * GK + q * 4 + lc;
+            double wv = 0.0;
+            if (k < K) {
+                double d = __ldg(kin + (k >> 1)) - lambda;
+                if (fabs(d) < dfloor) d = d < 0 ? -dfloor : dfloor;
+                wv = (k >= 2) ? 2.0 / d : (k == 0 ? 1.0 / d : 0.0);
+            }
+            w[q] = wv;
+        }
+        cp_wait<ST - 2>();
+        __syncthreads();
+        if (kt + ST - 1 < KT) load_stage((kt + ST - 1) % ST, kt + ST - 1);
+        cp_commit();
+        const double* As = gsm + (size_t)(kt % ST) * (BM + BN) * LDK + (wm0 + lr) * LDK + lc;
+        const double* Bs = gsm + (size_t)(kt % ST) * (BM + BN) * LDK + (BM + wn0 + lr) * LDK + lc;
+#pragma unroll
+        for (int k0 = 0; k0 < GK; k0 += 4) {
+            double af[FM], bf[FN];
+#pragma unroll
+            for (int i = 0; i < FM; ++i) af[i] = As[i * 8 * LDK + k0];
+#pragma unroll
+            for (int j = 0; j < FN; ++j) bf[j] = Bs[j * 8 * LDK + k0] * w[k0 / 4];
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) dmma(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+    }
+    cp_wait<0>();
+    double* dst = S + (size_t)blockIdx.z * M * M;
+#pragma unroll
+    for (int i = 0; i < FM; ++i) {
+        const int m = m0 + wm0 + i * 8 + lr;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < FN; ++j)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int n = n0 + wn0 + j * 8 + 2 * lc + h;
+                if (n < M) dst[(long)m * M + n] = acc[i][j][h];
+            }
+    }
+}
+
 }  // namespace tddft

@@ -163,10 +163,13 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // and used for both directions: 110 DMMAs per warp between barriers and ~0.14 bytes of L2->SM traffic per flop instead
 // of 0.375.  Row pitch FT_PITCH = 6 doubles and 108 rows per column make (row stride) = 8 mod 16 doubles, so both
 // fragment patterns (lanes over (i, j) for tau and over (j, i) for tau^T) spread over 8 distinct 8-byte banks: 4
-// wavefronts per load.  Results leave through shared memory so that every global access is a full 32-byte row.
+// wavefronts per load.  (Measured and rejected in round 2: storing tau with the two points of a 16-byte piece swapped in
+// alternate rows so that a half warp hits 16 different banks -- 2 wavefronts per load -- made the kernel 5 % slower, 352 vs
+// 333 ms: shared-memory wavefronts are not what limits it.)  Results leave through shared memory so that every global access
+// is a full 32-byte row.
 // Tile shapes: MT row tiles of 8 per warp, IR rows per column in a stage (= largest row block; IR = 4 mod 8 for the bank pattern).
 // The smaller shape leaves registers for the compiler to run fragment loads ahead of the DMMAs.
-struct FullShapeL { static constexpr int MT = 14, IR = 108; };
+struct FullShapeL { static constexpr int MT = 14, IR = 108; static constexpr int TMAX = 108; };
 struct FullShapeS { static constexpr int MT = 11, IR = 92; static constexpr int TMAX = 88; };
 constexpr int FT_P = 4;          // grid points (= warps) per CTA: two CTAs per SM, so one CTA's prologue/epilogue hides behind the other's DMMAs
 constexpr int FT_PPR = FT_P / 2; // 16-byte pieces per shared-memory row
@@ -175,7 +178,7 @@ constexpr int FT_JS = 8;         // columns per stage
 constexpr int FT_PF = 3;         // A fragments in flight ahead of the DMMAs (5 measured no better, copies interleaved with the DMMAs worse)
 template <int NK, class SH> struct FullCfg {
     static constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
-    static_assert((FT_IR * FT_PITCH) % 16 == 8 && FT_PITCH % 2 == 0, "fragment bank pattern");
+    static_assert((FT_IR * FT_PITCH) % 16 == 8 && FT_PITCH % 2 == 0 && FT_IR >= SH::TMAX, "fragment bank pattern");
     static constexpr int KB = 8 * NK;                                   // trial vectors per launch
     static constexpr int ROWS = FT_JS * FT_IR + FT_JS * KB;             // rows of one stage
     static constexpr int STAGE = ROWS * FT_PITCH;                       // doubles
@@ -379,7 +382,7 @@ static cudaError_t contract_full_launch(long nchunks, double* out, const double*
     contract_full_kernel<NK, DIAG, SH><<<(unsigned)(nchunks * (CHUNK / FT_P)), 32 * FT_P, smem, st>>>(out, a, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
     return cudaGetLastError();
 }
-int contract_full_max_tile() { return FullShapeL::IR; }
+int contract_full_max_tile() { return FullShapeL::TMAX; }
 int contract_full_small_tile() { return FullShapeS::TMAX; }
 template <class SH>
 static cudaError_t contract_full_shape(bool diag, long nchunks, double* o, const double* ap, const double* tau, int i0, int ti, int j0, int tj,
@@ -391,7 +394,7 @@ static cudaError_t contract_full_shape(bool diag, long nchunks, double* o, const
 }
 cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
                                  long ftot, long stot, long nr, double alpha, cudaStream_t st) {
-    if (ti > FullShapeL::IR || tj < 1 || ti < 1 || (diag && ti != tj)) return cudaErrorInvalidValue;
+    if (ti > FullShapeL::TMAX || tj < 1 || ti < 1 || (diag && ti != tj)) return cudaErrorInvalidValue;
     const long nchunks = (nr + CHUNK - 1) / CHUNK;
     for (int kb = 0; kb < kc; kb += 16) {
         const int kn = kc - kb < 16 ? kc - kb : 16;

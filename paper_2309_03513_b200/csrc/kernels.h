@@ -59,6 +59,10 @@ cudaError_t launch_lda_fxc(const double* rho_up, const double* rho_dn, long nr, 
 cudaError_t launch_gemm_nt(const double* A, long lda, const double* B, long ldb, int bgrp, long bstride_grp, double* C, long ldc,
                            int M, int N, long K, long wperiod, double cscale, int splits, double* partial, cudaStream_t st);
 int gemm_nt_tile_count(int M, int N);   // CTAs per k split of launch_gemm_nt (for choosing splits that fill the SMs)
+// S_b[u][u'] = <phi_u| (T - lam_b)^-1 |phi_u'> (Gamma inner product, |T - lam| floored at dfloor keeping sign) for nb shifts;
+// Phi [M][K] with K = 2 npwh reals, kin [npwh], lam device [nb], S [nb][M][M]  (reading A11b: projector-aware Davidson correction)
+cudaError_t launch_gram_shift(const double* Phi, long lda, int M, long K, const double* kin, const double* lam, int nb, double dfloor,
+                              double* S, cudaStream_t st);
 // C[m][n] += cscale * sum_k At[k][m] B[k][n];  C row m at  C + (m / cgrp)*cstride_grp + (m % cgrp)*ldc
 cudaError_t launch_gemm_tn_acc(const double* At, long ldat, const double* B, long ldb, double* C, long ldc, int cgrp,
                                long cstride_grp, int M, long N, int K, double cscale, cudaStream_t st);

@@ -73,3 +73,48 @@ def test_davidson_finds_the_lowest_roots_of_the_dense_matrix(mode):
     theta, X, it, res = davidson(P, 3, x0, mode=mode, tol=1e-8, max_subspace=30)
     assert np.max(np.abs(theta - exact[:3])) < 1e-10
     assert np.all(res <= 1e-8)
+
+
+@pytest.mark.parametrize("mode", [lv.SPIN_CONSERVING, lv.SPIN_FLIP])
+def test_projector_aware_correction_and_d_start_vectors(mode):
+    """Readings A11b / A11c: the projector-aware correction solves P_c (T - eps_v - theta) P_c t = r on range(P_c) exactly, the
+    start vectors are exact eigenvectors of D alone, and neither changes the converged roots (dense diagonalisation)."""
+    from oracle.davidson import d_start_vectors, precond_projector
+    lattice = [[4.0, 0, 0], [0.5, 4.2, 0], [0.3, -0.2, 4.5]]
+    grid, ecut = (6, 5, 4), 6.0
+    miller, g2 = lat.enumerate_half_sphere(lattice, ecut)
+    rng = np.random.default_rng(22)
+    psi = [inputs.orbitals(rng, n, g2, ecut) for n in (2, 2)]
+    eig = [inputs.eigenvalues(rng, 2) for _ in range(2)]
+    P = lv.Problem(lattice, grid, ecut, 2, psi, eig, 0.3)
+    # (i) the correction: apply P_c (T - lam) P_c to t block by block and recover r (r taken in range(P_c))
+    blocks = [(2, psi[0]), (2, psi[1])] if mode == lv.SPIN_CONSERVING else [(2, psi[1])]
+    r = inputs.trial_vectors(rng, blocks, 1)[0]
+    theta = 0.37
+    t = precond_projector(P, r, theta, mode)
+    assert np.linalg.norm(P.project_vector(t, mode) - t) < 1e-12 * np.linalg.norm(t)          # t lives in range(P_c)
+    so = [0, 1] if mode == lv.SPIN_CONSERVING else [0]
+    back, o = [], 0
+    for b, s_occ in enumerate(so):
+        s_tgt = s_occ if mode == lv.SPIN_CONSERVING else 1
+        for v in range(2):
+            tv = t[o:o + P.npwh]
+            back.append(P.project_c((0.5 * P.g2 - P.eig[s_occ][v] - theta) * tv, s_tgt))
+            o += P.npwh
+    assert np.linalg.norm(np.concatenate(back) - r) < 1e-10 * np.linalg.norm(r)
+    # (ii) D-only eigenvectors: with alpha = 0 and no Hxc the operator is D and x0 are exact eigenvectors, ascending
+    P0 = lv.Problem(lattice, grid, ecut, 2, psi, eig, 0.0, use_hartree_fxc=False)
+    x0 = d_start_vectors(P0, 5, mode)
+    AX = P0.apply(x0, mode)
+    ev = [P0.vdot(x0[i], AX[i]) for i in range(5)]
+    for i in range(5):
+        assert np.linalg.norm(AX[i] - ev[i] * x0[i]) < 1e-10
+        assert P0.vdot(x0[i], x0[i]) == pytest.approx(1.0, abs=1e-12)
+    assert np.all(np.diff(ev) >= -1e-12)
+    exact0 = np.linalg.eigvalsh(dense_matrix(P0, mode))
+    assert np.allclose(ev, exact0[:5], atol=1e-10)
+    # (iii) the full solver with both readings finds the lowest roots of the dense matrix
+    H = dense_matrix(P, mode)
+    exact = np.linalg.eigvalsh(0.5 * (H + H.T))
+    th, X, it, res = davidson(P, 3, d_start_vectors(P, 6, mode), mode=mode, tol=1e-8, max_subspace=30, precond="projector")
+    assert np.max(np.abs(th - exact[:3])) < 1e-10 and np.all(res <= 1e-8)

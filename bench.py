@@ -182,7 +182,8 @@ def oracle_sample(cfg, P=None, X=None, n_pp=None):
             desc.append("%d of the %d pair potentials of column (spin %d, v %d): %.1f s" % (npp, P.nocc[s], s, v, tpp))
     t_vec = t_prep + t_cols
     return {
-        "value": 1.0 / t_vec, "unit": UNIT, "cores": int(_threads_used()), "kind": "oracle",
+        # the oracle's time is in its FFTs (numpy pocketfft, one thread); BLAS threads only touch the small projector dot products
+        "value": 1.0 / t_vec, "unit": UNIT, "cores": 1, "blas_threads_available": int(_threads_used()), "kind": "oracle",
         "sample": "oracle on the full %s configuration (numpy.fft backend): prepare of one trial vector (%.1f s) + %s; "
                   "scaled to one vector apply = prepare + (N_up + N_dn) columns (an extrapolation: %.0f s per vector apply)"
                   % (cfg["name"], t_prep, "; ".join(desc), t_vec),

@@ -77,7 +77,7 @@ static SArgs xpass_args(const tddft_ctx* c, int batch, int kind) {
     const int* n = c->hp.n;
     const long inner = c->fused ? c->hp.ncols[kind] : (long)n[1] * n[2];
     SArgs a{}; a.n = n[0]; a.stride = inner; a.inner = inner; a.nouter = 1; a.outer_stride = 0;
-    a.nr = work_stride(c, kind); a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc; a.variant = c->dev_variant;
+    a.nr = work_stride(c, kind); a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc;
     return a;
 }
 static ZArgs zpass_args(const tddft_ctx* c, int batch, int kind) {
@@ -587,8 +587,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->dav_max_subspace = opt->max_subspace; c->dav_max_iter = opt->max_iter; c->dav_tol = opt->tol;
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
             c->dav_block = opt->block; c->dav_precond = opt->precond; c->verbose = opt->verbose;
-            c->fused = opt->fft_path == 0 || opt->fft_path >= 2;      // >= 2: development variants of the fused kernels
-            c->dev_variant = opt->fft_path >= 2 ? opt->fft_path - 1 : 0;
+            c->fused = opt->fft_path == 0;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
             if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");
             if (opt->s_thr < 0 || opt->n_pairs_up < 0 || opt->n_pairs_dn < 0 || opt->n_ace_extra_up < 0 || opt->n_ace_extra_dn < 0)

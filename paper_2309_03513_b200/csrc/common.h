@@ -52,7 +52,6 @@ enum SMode { SM_FWD = 0, SM_INV = 1, SM_CONV = 2 /* forward, multiply by ktab, i
 struct SArgs {
     int n; long stride; long inner; long nouter; long outer_stride; long nr; int batch;
     const cplx* tw; cplx* work; const double* ktab;   // ktab [nr] real, same (scrambled) layout as work
-    int variant;           // development switch of the fused x pass (0 = default)
 };
 bool fft_size_supported(int n);
 cudaError_t launch_zpass(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st);

@@ -39,7 +39,6 @@ struct tddft_ctx {
     double workspace_gb = 0;
     int pair_tile = 0, fft_batch = 0;
     int num_sms = 148;
-    int dev_variant = 0;             // development switch for A/B measurements of kernel variants (0 in production)
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off
     int dav_max_subspace = 0, dav_max_iter = 0, dav_block = 0, dav_precond = 0, verbose = 0;
     double dav_tol = 0; const double* dav_x0 = nullptr; int dav_nx0 = 0;

@@ -6,8 +6,8 @@
 namespace tddft {
 
 // (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
-#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8)
-#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12)
+#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8) X(96, 100, 360, 1)
+#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12) X(96)
 
 // Launch policy, fixed after the round-1 measurements (profiles/r01g_summary.md, r01i_summary.md): persistent grids that walk
 // the units plane-major; L2 prefetch of the CTA's next work-grid plane (inverse kernels) but not of orbital planes (they are
@@ -54,20 +54,20 @@ static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArg
     return cudaErrorInvalidValue;
 }
 
-template <int NX, bool LIT>
+template <int NX>
 static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     static_assert(Two<NX>::ok, "fused x pass needs a two-stage plan");
     constexpr size_t smem = XCfg<NX>::SMEM;
     static int resident_d[kMaxDevices] = {0};
     const int dev = current_device();
     if (!resident_d[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(xpass_kernel<NX, SM_FWD, LIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_INV, LIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_CONV, LIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(xpass_kernel<NX, SM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_kernel<NX, SM_CONV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         int sms = 0, per_sm = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_kernel<NX, SM_CONV, LIT>, XCfg<NX>::NTHR, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_kernel<NX, SM_CONV>, XCfg<NX>::NTHR, smem);
         resident_d[dev] = sms * (per_sm > 0 ? per_sm : 1);
     }
     const int resident = resident_d[dev];
@@ -84,9 +84,9 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     }
     dim3 grid(tiles, (unsigned)best_gy);
     constexpr int NT = XCfg<NX>::NTHR;
-    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD, LIT><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
-    else if (mode == SM_INV) xpass_kernel<NX, SM_INV, LIT><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
-    else xpass_kernel<NX, SM_CONV, LIT><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
     return cudaGetLastError();
 }
 
@@ -107,7 +107,7 @@ cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, con
     return cudaErrorInvalidValue;
 }
 cudaError_t launch_xpass(int mode, const SArgs& a, cudaStream_t st) {
-#define X(N) if (a.n == N) return a.variant ? xpass_launch<N, false>(mode, a, st) : xpass_launch<N, true>(mode, a, st);
+#define X(N) if (a.n == N) return xpass_launch<N>(mode, a, st);
     TD_FOR_EACH_XLEN(X)
 #undef X
     return cudaErrorInvalidValue;

@@ -454,13 +454,15 @@ template <int NX> struct XCfg {
     static constexpr int R1 = Two<NX>::R1, R2 = Two<NX>::R2;
     static constexpr int G = R1 > R2 ? R1 : R2;
     static constexpr int NTHR = G * XW;
+    static constexpr int MINB = G > 9 ? 2 : 3;          // CTAs per SM the registers are budgeted for (radix-12 butterflies need more)
     static constexpr size_t SMEM = sizeof(cplx) * NX * XW;
 };
 // Twiddles: the residue / block index g = tid / XW is the warp index (XW = 32), so every stage dispatches on g to a
 // body whose twiddles exp(-2 pi i g k / NX) are literals (mul_tw folds +-1, +-i and the octants): no twiddle registers
-// or loads, 3 CTAs per SM.  The barriers stay outside the per-warp bodies.
-template <int NX, int MODE, bool LIT>
-__global__ void __launch_bounds__(XCfg<NX>::NTHR, 3) xpass_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
+// or loads, 3 CTAs per SM.  The barriers stay outside the per-warp bodies.  (One generic body with warp-uniform twiddle loads
+// is nine times less code and was measured in round 2: same speed within noise, 632.8 vs 630.6 ms of S4; not kept.)
+template <int NX, int MODE>
+__global__ void __launch_bounds__(XCfg<NX>::NTHR, XCfg<NX>::MINB) xpass_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
                                                                  const cplx* __restrict__ tw_g, const double* __restrict__ ktab, int hint) {
     const unsigned long long pol = l2_policy(hint);
     constexpr int R1 = XCfg<NX>::R1, R2 = XCfg<NX>::R2;
@@ -475,19 +477,7 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, 3) xpass_kernel(cplx* __restri
     }
     for (int b = blockIdx.y; b < batch; b += gridDim.y) {
         cplx* gcol = work + (long)b * nr + col;
-        if (!LIT && (MODE == SM_FWD || MODE == SM_CONV)) {
-            if (g < R2) {       // stage R1 forward of residue g: rows g + R2*r, twiddle w^(g k) after (warp-uniform loads)
-                cplx x[R1];
-#pragma unroll
-                for (int r = 0; r < R1; ++r) x[r] = live ? ld_pol(gcol + (long)(g + R2 * r) * inner, pol) : make_double2(0.0, 0.0);
-                Dft<R1, false>::run(x);
-                sm[g * XW + c] = x[0];
-#pragma unroll
-                for (int k = 1; k < R1; ++k) sm[(g + R2 * k) * XW + c] = cmul(x[k], __ldg(tw_g + g * k));
-            }
-            __syncthreads();
-        }
-        if (LIT && (MODE == SM_FWD || MODE == SM_CONV)) {
+        if (MODE == SM_FWD || MODE == SM_CONV) {
             static_for<0, R2>([&](auto g_) {       // stage R1 forward of residue g: rows g + R2*r, twiddle after
                 constexpr int GI = decltype(g_)::value;
                 if (g == GI) {
@@ -528,21 +518,7 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, 3) xpass_kernel(cplx* __restri
                 for (int i = 0; i < R2; ++i) sm[(g * R2 + i) * XW + c] = x[i];
             }
         }
-        if (!LIT && MODE != SM_FWD) {
-            __syncthreads();
-            if (g < R2) {
-                cplx x[R1];
-                x[0] = sm[g * XW + c];
-#pragma unroll
-                for (int k = 1; k < R1; ++k) x[k] = cmulc(sm[(g + R2 * k) * XW + c], __ldg(tw_g + g * k));
-                Dft<R1, true>::run(x);
-                if (live) {
-#pragma unroll
-                    for (int r = 0; r < R1; ++r) st_pol(gcol + (long)(g + R2 * r) * inner, x[r], pol);
-                }
-            }
-        }
-        if (LIT && MODE != SM_FWD) {
+        if (MODE != SM_FWD) {
             __syncthreads();
             static_for<0, R2>([&](auto g_) {       // stage R1 inverse of residue g: conjugate twiddle, butterfly, natural order out
                 constexpr int GI = decltype(g_)::value;

@@ -120,7 +120,7 @@ def test_apply_config3_sampled_columns(mode):
 
 
 @pytest.mark.parametrize("grid,lattice,ecut,nocc,nvec", [
-    # the three-stage plans of the general pass kernels, never reached by the smaller grids: 96 = 6*4*4, 100 = 10*10, 108 = 3*6*6,
+    # the large plans, never reached by the smaller grids: 96 = 12*8, 100 = 10*10 (fused kernels and general path), 108 = 3*6*6,
     # 128 = 8*4*4 (fft_core.cuh); the shapes of BASELINE.json configs[3] (hexagonal) and [4] and of the 60 Ry workload
     ((96, 96, 100), [[12.0, 0, 0], [-6.0, 12.0 * 0.8660254037844386, 0], [0, 0, 8.0]], 5.0, (4, 3), 2),
     ((108, 108, 108), [[9.0, 0, 0], [0, 9.0, 0], [0, 0, 9.0]], 8.0, (4, 3), 2),
@@ -128,6 +128,28 @@ def test_apply_config3_sampled_columns(mode):
 ])
 def test_apply_large_fft_plans(grid, lattice, ecut, nocc, nvec):
     case = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid))      # oracle with its own radix FFT
+    general = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid), oracle=False, fft_path=1) if grid == (96, 96, 100) else None
     for mode in (0, 1):
         X = case.trial(nvec, mode)
-        assert rel_fro(case.gpu_apply(X, mode), case.oracle.apply(X, mode)) < TOL
+        ref = case.oracle.apply(X, mode)
+        assert rel_fro(case.gpu_apply(X, mode), ref) < TOL                 # 96 x 96 x 100: the fused plane / x kernels (1 CTA per SM)
+        if general is not None:
+            assert rel_fro(general.gpu_apply(X, mode), ref) < TOL          # and the general pass kernels on the same shape
+
+
+def test_apply_config4_shape_with_block_at_a_time_plan():
+    # the lattice, grid and cutoff of BASELINE.json configs[3] (hexagonal 4H-SiC shaped cell, 96 x 96 x 100, 20 Ry) with fewer
+    # orbitals, under a workspace cap that forces the plan of the full configuration: one spin block resident at a time, trial
+    # vectors in chunks (tau recomputed per chunk), small tiles.  Sampled columns + invariants, as at the full sizes.
+    from paper_2309_03513_b200 import binding as b
+    import synthetic_inputs as inputs
+    cfg = inputs.config(4)
+    case = Case(cfg["lattice"], cfg["grid"], cfg["ecut"], 2, (40, 38), cfg["alpha"], cfg["seed"], envelope=True, ortho="qr",
+                fft_backend="numpy", workspace_gb=3.2)
+    X = case.trial(3, 0)
+    got = case.gpu_apply(X, 0)
+    st = b.tddft_get_stats(case.ctx())
+    assert st["k_chunk"] < 3 or st["blocks_resident"] == 0 or st["pair_tile"] < 40, st
+    samples = [(0, 0, 0), (0, 1, 37), (2, 0, 39), (2, 1, 16), (1, 0, 17)]
+    assert _sampled_columns(case, X, got, 0, samples) < TOL
+    _invariants(case, X, got, 0)

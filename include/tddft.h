@@ -98,6 +98,10 @@ typedef struct {
   int ace;
   const double* psi_ace_up; int n_ace_extra_up;
   const double* psi_ace_dn; int n_ace_extra_dn;
+  /* Fused FFT path: launches whose frequency-space work grids are smaller than this many MB leave them to the normal L2
+   * replacement policy (they are read back by the next kernel of the pipeline); larger launches stream them with an
+   * evict-first hint so that they do not displace the orbital planes.  <= 0: default 48. */
+  double work_l2_mb;
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,

@@ -73,11 +73,13 @@ static SArgs ypass_args(const tddft_ctx* c, int batch) {
 // columns of the transform's kind (plan.h: KIND_PROD = products of two sphere functions, KIND_SPHERE = sphere functions).
 enum { KIND_PROD = 0, KIND_SPHERE = 1 };
 static long work_stride(const tddft_ctx* c, int kind) { return c->fused ? (long)c->hp.n[0] * c->hp.ncols[kind] : c->hp.nr; }
+static int work_hint(const tddft_ctx* c, int batch, int kind) { return (double)batch * (double)work_stride(c, kind) * sizeof(cplx) > c->work_l2_mb * 1048576.0 ? 1 : 0; }
 static SArgs xpass_args(const tddft_ctx* c, int batch, int kind) {
     const int* n = c->hp.n;
     const long inner = c->fused ? c->hp.ncols[kind] : (long)n[1] * n[2];
     SArgs a{}; a.n = n[0]; a.stride = inner; a.inner = inner; a.nouter = 1; a.outer_stride = 0;
     a.nr = work_stride(c, kind); a.batch = batch; a.tw = c->d_tw[0]; a.work = c->d_work; a.ktab = c->d_vc;
+    a.whint = work_hint(c, batch, kind);
     return a;
 }
 static ZArgs zpass_args(const tddft_ctx* c, int batch, int kind) {
@@ -85,6 +87,7 @@ static ZArgs zpass_args(const tddft_ctx* c, int batch, int kind) {
     ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.tw2 = c->d_tw[1]; a.work = c->d_work;
     a.lscale = 1.0; a.sscale = 1.0;
     a.cmap = c->d_cmap[kind]; a.ncols = c->hp.ncols[kind]; a.wstride = work_stride(c, kind);
+    a.whint = work_hint(c, batch, kind);
     return a;
 }
 
@@ -588,6 +591,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
             c->dav_block = opt->block; c->dav_precond = opt->precond; c->verbose = opt->verbose;
             c->fused = opt->fft_path == 0;
+            if (opt->work_l2_mb > 0) c->work_l2_mb = opt->work_l2_mb;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
             if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");
             if (opt->s_thr < 0 || opt->n_pairs_up < 0 || opt->n_pairs_dn < 0 || opt->n_ace_extra_up < 0 || opt->n_ace_extra_dn < 0)

@@ -44,6 +44,7 @@ struct ZArgs {
     int chunked; long fbase; long ftotal;
     // fused path only: pruned layout of the work grids (plan.h): column map, live columns, grid stride in `work`
     const int* cmap; int ncols; long wstride;
+    int whint;             // L2 policy of the work-grid stream: 1 = evict first, 0 = normal (the launch's work grids fit in L2)
 };
 constexpr int CHUNK = 32;
 inline long chunked_elems(long nfun, long nr) { return (nr + CHUNK - 1) / CHUNK * CHUNK * nfun; }
@@ -52,6 +53,7 @@ enum SMode { SM_FWD = 0, SM_INV = 1, SM_CONV = 2 /* forward, multiply by ktab, i
 struct SArgs {
     int n; long stride; long inner; long nouter; long outer_stride; long nr; int batch;
     const cplx* tw; cplx* work; const double* ktab;   // ktab [nr] real, same (scrambled) layout as work
+    int whint;             // fused path: L2 policy of the work-grid stream (see ZArgs)
 };
 bool fft_size_supported(int n);
 cudaError_t launch_zpass(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st);

@@ -37,6 +37,7 @@ struct tddft_ctx {
     const double* vloc[2] = {nullptr, nullptr};
     cudaStream_t stream = nullptr;
     double workspace_gb = 0;
+    double work_l2_mb = 48.0;        // launches with smaller work grids keep them under the normal L2 policy
     int pair_tile = 0, fft_batch = 0;
     int num_sms = 148;
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off

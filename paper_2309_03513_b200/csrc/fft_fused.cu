@@ -42,8 +42,8 @@ static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t 
 template <int NY, int NZ, int NTHR, int MINB>
 static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
     const int hint = kStreamHint;
-    LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols, hint};
-    StoreWorkC sw{a.work, a.wstride, a.cmap, a.ncols, hint};
+    LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols, a.whint};
+    StoreWorkC sw{a.work, a.wstride, a.cmap, a.ncols, a.whint};
     const BatchLayout lay{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr};
     if (!inverse) {
         if (lkind == ZL_PAIR) return plane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.phi2 ? a.phi2 : a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
@@ -84,9 +84,9 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     }
     dim3 grid(tiles, (unsigned)best_gy);
     constexpr int NT = XCfg<NX>::NTHR;
-    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
-    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
-    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, kStreamHint);
+    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
     return cudaGetLastError();
 }
 

@@ -139,272 +139,7 @@ cudaError_t launch_out_init(const double* phi, const double* V, const double* vl
     return cudaGetLastError();
 }
 
-// S5: out[(i0+i)*kc+k][r] -= alpha * sum_j tau_ij(r) a[(j0+j)*kc+k][r]   (Eq. 6).
-// Per grid point this is a (ti x tj)(tj x kc) product whose matrices differ at every r: a batch of N_r small GEMMs,
-// run on the FP64 tensor pipe (mma.sync.m8n8k4.f64).  All real-space batches (tau, a, out) use the chunked layout
-// [nr/32][function][32].
-__device__ __forceinline__ void dmma884k(double& c0, double& c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// ------------------------------------------------------------------------------------------------------
-// S5, register-resident tiles.  One warp owns ONE grid point and keeps the whole row block of the tile in registers:
-// the accumulators of out[I] (up to 112 rows x 16 trial vectors = 56 doubles per lane) and, for off-diagonal tiles,
-// the B fragments of a[I] (54 doubles) that the transposed product out[J] += tau^T a[I] needs.  The CTA (FT_P = 4 warps =
-// 4 consecutive points, two CTAs per SM) sweeps the columns of the tile 8 at a time through a double-buffered cp.async
-// stage (tau[all i][8 j] and a[8 j][16 k], 32-byte rows padded to 48 bytes); every tau element is loaded into the SM once
-// and used for both directions: 110 DMMAs per warp between barriers and ~0.14 bytes of L2->SM traffic per flop instead
-// of 0.375.  Row pitch FT_PITCH = 6 doubles and 108 rows per column make (row stride) = 8 mod 16 doubles, so both
-// fragment patterns (lanes over (i, j) for tau and over (j, i) for tau^T) spread over 8 distinct 8-byte banks: 4
-// wavefronts per load.  (Measured and rejected in round 2: storing tau with the two points of a 16-byte piece swapped in
-// alternate rows so that a half warp hits 16 different banks -- 2 wavefronts per load -- made the kernel 5 % slower, 352 vs
-// 333 ms: shared-memory wavefronts are not what limits it.)  Results leave through shared memory so that every global access
-// is a full 32-byte row.
-// Tile shapes: MT row tiles of 8 per warp, IR rows per column in a stage (= largest row block; IR = 4 mod 8 for the bank pattern).
-// The smaller shape leaves registers for the compiler to run fragment loads ahead of the DMMAs.
-struct FullShapeL { static constexpr int MT = 14, IR = 108; static constexpr int TMAX = 108; };
-struct FullShapeS { static constexpr int MT = 11, IR = 92; static constexpr int TMAX = 88; };
-constexpr int FT_P = 4;          // grid points (= warps) per CTA: two CTAs per SM, so one CTA's prologue/epilogue hides behind the other's DMMAs
-constexpr int FT_PPR = FT_P / 2; // 16-byte pieces per shared-memory row
-constexpr int FT_PITCH = FT_P + 2;   // doubles per shared-memory row (rows stay 16-byte aligned)
-constexpr int FT_JS = 8;         // columns per stage
-constexpr int FT_PF = 3;         // A fragments in flight ahead of the DMMAs (5 measured no better, copies interleaved with the DMMAs worse)
-template <int NK, class SH> struct FullCfg {
-    static constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
-    static_assert((FT_IR * FT_PITCH) % 16 == 8 && FT_PITCH % 2 == 0 && FT_IR >= SH::TMAX, "fragment bank pattern");
-    static constexpr int KB = 8 * NK;                                   // trial vectors per launch
-    static constexpr int ROWS = FT_JS * FT_IR + FT_JS * KB;             // rows of one stage
-    static constexpr int STAGE = ROWS * FT_PITCH;                       // doubles
-    static constexpr int FLUSH = FT_JS * KB * FT_PITCH;                 // doubles (two of them: products and prefetched out[J] rows)
-    static constexpr size_t SMEM = sizeof(double) * (2 * STAGE + 2 * FLUSH);
-    static_assert(FT_MT * 8 * KB * FT_PITCH <= 2 * STAGE, "the epilogue stages the row block through the two stage buffers");
-};
-template <int NK, bool DIAG, class SH>
-__global__ void __launch_bounds__(32 * FT_P, 2)
-contract_full_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau,
-                     int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
-    extern __shared__ __align__(16) double sm[];
-    using C = FullCfg<NK, SH>;
-    constexpr int FT_MT = SH::MT, FT_IR = SH::IR;
-    constexpr int KB = C::KB, IR = FT_IR, PITCH = FT_PITCH, JS = FT_JS, PPR = FT_PPR;
-    constexpr int NTHR = 32 * FT_P, RSTEP = NTHR / PPR;     // rows covered by one pass of the CTA over 16-byte pieces
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, lr = lane >> 2, lc = lane & 3;
-    const long chunk = blockIdx.x / (CHUNK / FT_P);
-    const int pt0 = (int)(blockIdx.x % (CHUNK / FT_P)) * FT_P;
-    const double* tau_c = tau + chunk * stot * CHUNK + pt0;
-    const double* a_c = a + chunk * ftot * CHUNK + pt0;
-    double* out_c = out + chunk * ftot * CHUNK + pt0;
-    const int piece2 = (tid % PPR) * 2, rsub = tid / PPR;    // this thread's 16-byte piece of rows rsub, rsub + RSTEP, ...
-    double* fl = sm + 2 * C::STAGE;                          // products of the transposed direction, [8 j * KB][PITCH]
-    double* ojs = fl + C::FLUSH;                             // the out[J] rows they are subtracted from, prefetched by cp.async
-
-    // ---- prologue: a[I] -> shared memory (coalesced) -> B fragments of the transposed product
-    double breg[DIAG ? 1 : IR / 4][NK];
-    if (!DIAG) {
-        for (int row = rsub; row < IR * KB; row += RSTEP) {
-            const int i = row / KB, kk = row - i * KB;
-            double* dst = sm + row * PITCH + piece2;
-            if (i < ti && kk < kn) cp_async16(dst, a_c + ((long)(i0 + i) * kc + kk) * CHUNK + piece2);
-            else *(double2*)dst = make_double2(0.0, 0.0);
-        }
-        cp_async_commit();
-        cp_async_wait<0>();
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < IR / 4; ++q)
-#pragma unroll
-            for (int n = 0; n < NK; ++n) breg[q][n] = sm[((q * 4 + lc) * KB + n * 8 + lr) * PITCH + w];
-        __syncthreads();
-    }
-    // Stage loader.  tau part: a group of 8*PPR lanes copies the pieces of the 8 columns of one row i; rows advance by a
-    // constant, so a copy costs a pointer increment.  a part: 8*KB rows spread over the CTA.
-    constexpr int LPR = 8 * PPR, RPW = 32 / LPR, ISTEP = FT_P * RPW;
-    const int ljj = (lane % LPR) / PPR, lp2 = (lane % PPR) * 2, li0 = w * RPW + lane / LPR;
-    auto load_stage = [&](int buf, int js) {
-        double* base = sm + buf * C::STAGE;
-        const int col = js * JS + ljj;
-        double* dst = base + (ljj * IR + li0) * PITCH + lp2;
-        if (col < tj) {
-            if (DIAG) {
-#pragma unroll 2
-                for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH) {
-                    if (i < ti) {
-                        const int lo = min(i, col), hi = max(i, col);
-                        cp_async16(dst, tau_c + (long)(lo * (2 * tj - lo + 1) / 2 + (hi - lo)) * CHUNK + lp2);     // slots fit 32 bits
-                    } else *(double2*)dst = make_double2(0.0, 0.0);
-                }
-            } else {
-                const double* src = tau_c + ((long)li0 * tj + col) * CHUNK + lp2;
-                const long sstep = (long)ISTEP * tj * CHUNK;
-#pragma unroll 2
-                for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH, src += sstep) {
-                    if (i < ti) cp_async16(dst, src);
-                    else *(double2*)dst = make_double2(0.0, 0.0);
-                }
-            }
-        } else {
-            for (int i = li0; i < IR; i += ISTEP, dst += ISTEP * PITCH) *(double2*)dst = make_double2(0.0, 0.0);
-        }
-#pragma unroll
-        for (int e = 0; e < (JS * KB + RSTEP - 1) / RSTEP; ++e) {
-            const int rr = rsub + e * RSTEP;
-            if (rr < JS * KB) {
-                const int jj = rr / KB, kk = rr - jj * KB, cj = js * JS + jj;
-                double* d2 = base + (JS * IR + rr) * PITCH + piece2;
-                if (cj < tj && kk < kn) cp_async16(d2, a_c + ((long)(j0 + cj) * kc + kk) * CHUNK + piece2);
-                else *(double2*)d2 = make_double2(0.0, 0.0);
-            }
-        }
-    };
-    constexpr int NFL = (JS * KB + RSTEP - 1) / RSTEP;      // rows of out[J] per thread and stage
-    double acc[FT_MT][NK][2];
-#pragma unroll
-    for (int m = 0; m < FT_MT; ++m)
-#pragma unroll
-        for (int n = 0; n < NK; ++n) { acc[m][n][0] = 0.0; acc[m][n][1] = 0.0; }
-    const int nst = (tj + JS - 1) / JS;
-    load_stage(0, 0);
-    cp_async_commit();
-    for (int js = 0; js < nst; ++js) {
-        cp_async_wait<0>();
-        __syncthreads();                 // stage js has landed for everyone; stage js-1 and its flush are consumed
-        if (!DIAG) {                     // rows of out[J] this thread updates after the transposed product: fetched behind the DMMAs
-#pragma unroll
-            for (int e = 0; e < NFL; ++e) {
-                const int row = rsub + e * RSTEP, jj = row / KB, kk = row - jj * KB, col = js * JS + jj;
-                if (row < JS * KB && col < tj && kk < kn) cp_async16(ojs + row * PITCH + piece2, out_c + ((long)(j0 + col) * kc + kk) * CHUNK + piece2);
-            }
-        }
-        cp_async_commit();
-        if (js + 1 < nst) load_stage((js + 1) & 1, js + 1);
-        cp_async_commit();
-        const double* S = sm + (js & 1) * C::STAGE + w;
-        // direction 1: out[i][k] += sum_j tau[i][j] a[j][k]
-#pragma unroll
-        for (int s = 0; s < JS / 4; ++s) {
-            double bf[NK];
-#pragma unroll
-            for (int n = 0; n < NK; ++n) bf[n] = S[(JS * IR + (s * 4 + lc) * KB + n * 8 + lr) * PITCH];
-            // the A fragments run FT_PF tiles ahead of the DMMAs that use them (explicit rotation: the compiler does not
-            // move loads across the asm statements)
-            const double* Ap = S + ((s * 4 + lc) * IR + lr) * PITCH;
-            double afq[FT_PF];
-#pragma unroll
-            for (int m = 0; m < FT_PF; ++m) afq[m] = Ap[m * 8 * PITCH];
-#pragma unroll
-            for (int m = 0; m < FT_MT; ++m) {
-                const double af = afq[m % FT_PF];
-                if (m + FT_PF < FT_MT) afq[m % FT_PF] = Ap[(m + FT_PF) * 8 * PITCH];
-#pragma unroll
-                for (int n = 0; n < NK; ++n) dmma884k(acc[m][n][0], acc[m][n][1], af, bf[n]);
-            }
-        }
-        if (!DIAG) {
-            // direction 2: out[j][k] += sum_i tau[i][j] a[i][k], the 8 columns of this stage
-            double acc2[NK][2];
-#pragma unroll
-            for (int n = 0; n < NK; ++n) { acc2[n][0] = 0.0; acc2[n][1] = 0.0; }
-            const double* Atp = S + (lr * IR + lc) * PITCH;
-            double atq[FT_PF];
-#pragma unroll
-            for (int q = 0; q < FT_PF; ++q) atq[q] = Atp[q * 4 * PITCH];
-#pragma unroll
-            for (int q = 0; q < IR / 4; ++q) {
-                const double af = atq[q % FT_PF];
-                if (q + FT_PF < IR / 4) atq[q % FT_PF] = Atp[(q + FT_PF) * 4 * PITCH];
-#pragma unroll
-                for (int n = 0; n < NK; ++n) dmma884k(acc2[n][0], acc2[n][1], af, breg[q][n]);
-            }
-#pragma unroll
-            for (int n = 0; n < NK; ++n) {
-                fl[(lr * KB + n * 8 + 2 * lc) * PITCH + w] = acc2[n][0];
-                fl[(lr * KB + n * 8 + 2 * lc + 1) * PITCH + w] = acc2[n][1];
-            }
-            cp_async_wait<1>();          // this thread's out[J] pieces (the group before the next stage's copies)
-            __syncthreads();
-#pragma unroll
-            for (int e = 0; e < NFL; ++e) {
-                const int row = rsub + e * RSTEP, jj = row / KB, kk = row - jj * KB, col = js * JS + jj;
-                if (row < JS * KB && col < tj && kk < kn) {
-                    const double2 d = *(const double2*)(fl + row * PITCH + piece2);
-                    const double2 o = *(const double2*)(ojs + row * PITCH + piece2);
-                    *(double2*)(out_c + ((long)(j0 + col) * kc + kk) * CHUNK + piece2) = make_double2(fma(-alpha, d.x, o.x), fma(-alpha, d.y, o.y));
-                }
-            }
-        }
-    }
-    // ---- epilogue: out[I] -= alpha * acc through shared memory (full rows)
-    __syncthreads();
-#pragma unroll
-    for (int m = 0; m < FT_MT; ++m)
-#pragma unroll
-        for (int n = 0; n < NK; ++n) {
-            sm[((m * 8 + lr) * KB + n * 8 + 2 * lc) * PITCH + w] = acc[m][n][0];
-            sm[((m * 8 + lr) * KB + n * 8 + 2 * lc + 1) * PITCH + w] = acc[m][n][1];
-        }
-    __syncthreads();
-    constexpr int EB = 14;               // rows in flight per thread: the loads of a batch are issued before its stores
-    for (int row0 = rsub; row0 < ti * KB; row0 += EB * RSTEP) {
-        double2 o[EB]; double* p[EB];
-#pragma unroll
-        for (int e = 0; e < EB; ++e) {
-            const int row = row0 + e * RSTEP, i = row / KB, kk = row - i * KB;
-            p[e] = (row < ti * KB && kk < kn) ? out_c + ((long)(i0 + i) * kc + kk) * CHUNK + piece2 : nullptr;
-            o[e] = p[e] ? *(const double2*)p[e] : make_double2(0.0, 0.0);
-        }
-#pragma unroll
-        for (int e = 0; e < EB; ++e) {
-            if (p[e]) {
-                const double2 d = *(const double2*)(sm + (row0 + e * RSTEP) * PITCH + piece2);
-                *(double2*)p[e] = make_double2(fma(-alpha, d.x, o[e].x), fma(-alpha, d.y, o[e].y));
-            }
-        }
-    }
-}
-template <int NK, bool DIAG, class SH>
-static cudaError_t contract_full_launch(long nchunks, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj,
-                                        int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    constexpr size_t smem = FullCfg<NK, SH>::SMEM;
-    static bool attr_done[kMaxDevices] = {false};
-    const int dev = current_device();
-    if (!attr_done[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(contract_full_kernel<NK, DIAG, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done[dev] = true;
-    }
-    contract_full_kernel<NK, DIAG, SH><<<(unsigned)(nchunks * (CHUNK / FT_P)), 32 * FT_P, smem, st>>>(out, a, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha);
-    return cudaGetLastError();
-}
-int contract_full_max_tile() { return FullShapeL::TMAX; }
-int contract_full_small_tile() { return FullShapeS::TMAX; }
-template <class SH>
-static cudaError_t contract_full_shape(bool diag, long nchunks, double* o, const double* ap, const double* tau, int i0, int ti, int j0, int tj,
-                                       int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    if (kn > 8) return diag ? contract_full_launch<2, true, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                            : contract_full_launch<2, false, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-    return diag ? contract_full_launch<1, true, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                : contract_full_launch<1, false, SH>(nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-}
-cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
-                                 long ftot, long stot, long nr, double alpha, cudaStream_t st) {
-    if (ti > FullShapeL::TMAX || tj < 1 || ti < 1 || (diag && ti != tj)) return cudaErrorInvalidValue;
-    const long nchunks = (nr + CHUNK - 1) / CHUNK;
-    for (int kb = 0; kb < kc; kb += 16) {
-        const int kn = kc - kb < 16 ? kc - kb : 16;
-        double* o = out + (long)kb * CHUNK; const double* ap = a + (long)kb * CHUNK;
-        cudaError_t e = ti <= FullShapeS::TMAX ? contract_full_shape<FullShapeS>(diag, nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st)
-                                               : contract_full_shape<FullShapeL>(diag, nchunks, o, ap, tau, i0, ti, j0, tj, kc, kn, ftot, stot, alpha, st);
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
-}
+// S5 (the exchange contraction of Eq. 6) lives in contract.cu.
 
 // ------------------------------------------------------------------------------------------------------
 // V[kk][r] = f[r] * d[kk][r]: the spin-flip K1e potential f^SF * drho^SF (Eq. 24)

@@ -250,6 +250,7 @@ def main():
     ap.add_argument("--fft-path", type=int, default=0)
     ap.add_argument("--workspace-gb", type=float, default=0.0)
     ap.add_argument("--work-l2-mb", type=float, default=0.0)
+    ap.add_argument("--tile-width", type=int, default=0)
     ap.add_argument("--davidson", type=int, default=0, help="also run tddft_davidson for this many roots (not timed into `value`)")
     ap.add_argument("--max-iter", type=int, default=0)
     ap.add_argument("--precond", type=int, default=0)
@@ -287,7 +288,7 @@ def main():
     d_psi = [torch.from_numpy(p).cuda() for p in inp["psi"]]
     opts = {}
     for k, v in (("pair_tile", args.pair_tile), ("fft_batch", args.fft_batch), ("max_iter", args.max_iter), ("fft_path", args.fft_path),
-                 ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("precond", args.precond), ("verbose", args.verbose)):
+                 ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("tile_width", args.tile_width), ("precond", args.precond), ("verbose", args.verbose)):
         if v:
             opts[k] = v
     ctx = b.tddft_init(cfg["lattice"], cfg["grid"], cfg["ecut"], cfg["nspin"], cfg["nocc"], d_psi[0],
@@ -433,7 +434,7 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": list(cfg["grid"]), "nocc": list(cfg["nocc"]), "nvec": nvec,
                    "mode": ["spin_conserving", "spin_flip_up_down", "spin_flip_down_up"][mode], "alpha": cfg["alpha"],
-                   "pair_tile": st["pair_tile"], "k_chunk": st["k_chunk"], "blocks_resident": st["blocks_resident"],
+                   "pair_tile": st["pair_tile"], "tile_width": st["tile_width"], "k_chunk": st["k_chunk"], "blocks_resident": st["blocks_resident"],
                    "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": "images x%d" % world},
         "block_applies_per_s": value / nvec,
         "pair_ffts_per_s": (world * pairs_per_step / (s4_ms * 1e-3)) if s4_ms > 0 else None,

@@ -102,6 +102,8 @@ typedef struct {
    * replacement policy (they are read back by the next kernel of the pipeline); larger launches stream them with an
    * evict-first hint so that they do not displace the orbital planes.  <= 0: default 48. */
   double work_l2_mb;
+  int tile_width;           /* most columns of an off-diagonal tile of the exchange loop (rounded down to a multiple of the tile edge);
+                             * <= 0 = as wide as the workspace allows */
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,
@@ -170,6 +172,7 @@ typedef struct {
   int pair_tile;  /* tile edge of the last apply */
   int k_chunk;    /* trial vectors processed together (< nvec: the pair potentials were recomputed per chunk) */
   int blocks_resident; /* 1: the real-space functions of all spin blocks were resident; 0: one spin block at a time */
+  int tile_width;      /* columns of an off-diagonal tile of the last apply (a multiple of pair_tile) */
 } tddft_stats;
 int tddft_set_timing(tddft_ctx* ctx, int enabled); /* stage timing with CUDA events (adds synchronisation) */
 int tddft_get_stats(const tddft_ctx* ctx, tddft_stats* out);

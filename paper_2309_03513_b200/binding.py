@@ -37,7 +37,7 @@ class tddft_options(C.Structure):
         ("pair_list_up", C.c_void_p), ("n_pairs_up", C.c_long), ("pair_list_dn", C.c_void_p), ("n_pairs_dn", C.c_long),
         ("ace", C.c_int), ("psi_ace_up", C.c_void_p), ("n_ace_extra_up", C.c_int),
         ("psi_ace_dn", C.c_void_p), ("n_ace_extra_dn", C.c_int),
-        ("work_l2_mb", C.c_double),
+        ("work_l2_mb", C.c_double), ("tile_width", C.c_int),
     ]
 
 
@@ -47,7 +47,7 @@ class tddft_stats(C.Structure):
                 ("ms_s5_contract", C.c_double), ("ms_s6_to_sphere", C.c_double), ("ms_s8_project", C.c_double),
                 ("ms_s7_rotate_ace", C.c_double),
                 ("fft_batch", C.c_int), ("fft_path", C.c_int), ("pair_batch", C.c_int), ("pair_tile", C.c_int),
-                ("k_chunk", C.c_int), ("blocks_resident", C.c_int)]
+                ("k_chunk", C.c_int), ("blocks_resident", C.c_int), ("tile_width", C.c_int)]
 
 
 def load_library():

@@ -271,30 +271,33 @@ static void choose_subblock(int cap, int* si_out, int* sj_out) {
             if (cost < best) { best = cost; *si_out = si; *sj_out = sj; }
         }
 }
-int build_tiles(tddft_ctx* c, int spin, int T) {
+int build_tiles(tddft_ctx* c, int spin, int T, int W) {
     PairTiles& pt = c->tiles[spin];
     const int N = c->nocc[spin];
-    if (pt.T == T && pt.nocc == N && pt.d_pairs) return TDDFT_OK;
+    if (pt.T == T && pt.W == W && pt.nocc == N && pt.d_pairs) return TDDFT_OK;
     if (pt.d_pairs) cudaFree(pt.d_pairs);
     if (pt.d_pslot) cudaFree(pt.d_pslot);
     pt = PairTiles{};
-    pt.T = T; pt.nocc = N;
+    pt.T = T; pt.W = W; pt.nocc = N;
     // Processing order: sub-blocks of sbi rows x sbj columns (sbj even, sbi*sbj <= one launch of 2*fft_batch pairs), row-major
     // inside a sub-block.  A launch then multiplies sbi + sbj orbital grids (L2 resident) instead of ~2*fft_batch, and the two
     // pairs packed into one complex grid still share their first orbital.
     choose_subblock(2 * c->fft_batch, &pt.sbi, &pt.sbj);
     pt.batch_pairs = pt.sbi * pt.sbj;
     const std::vector<char>& mask = c->mask[spin];      // near-sightedness truncation (Eq. 32 / explicit pair list); empty = all pairs
+    // Tiles: per row block bi the diagonal tile (T x T, packed triangle) and off-diagonal tiles of up to W columns (W a multiple
+    // of T chosen from the workspace: a wide tile keeps the row block's accumulators and a[I] in the contraction's registers over
+    // more columns, so a[I] / out[I] cross HBM once per W columns instead of once per T).
     const int nb = (N + T - 1) / T;
     std::vector<int2> pairs; std::vector<int> pslot;
     for (int bi = 0; bi < nb; ++bi)
-        for (int bj = bi; bj < nb; ++bj) {
+        for (int cj0 = bi * T; cj0 < N; cj0 += (cj0 == bi * T ? T : W)) {
             TileInfo t{};
-            t.i0 = bi * T; t.ti = std::min(T, N - t.i0); t.j0 = bj * T; t.tj = std::min(T, N - t.j0);
-            t.diag = bi == bj;
+            t.diag = cj0 == bi * T;
+            t.i0 = bi * T; t.ti = std::min(T, N - t.i0); t.j0 = cj0; t.tj = std::min(t.diag ? T : W, N - t.j0);
             t.pair_off = (long)pairs.size();
-            // tau slots (the contraction's layout): dense i*tj + j, or the packed upper triangle i(2 tj - i + 1)/2 + (j - i) on the diagonal
-            auto slot_of = [&](int i, int j) { return t.diag ? i * (2 * t.tj - i + 1) / 2 + (j - i) : i * t.tj + j; };
+            // tau slots (the contraction's layout): dense column-major j*ti + i, or the packed upper triangle i(2 tj - i + 1)/2 + (j - i) on the diagonal
+            auto slot_of = [&](int i, int j) { return t.diag ? i * (2 * t.tj - i + 1) / 2 + (j - i) : j * t.ti + i; };
             t.nslots = t.diag ? (long)t.ti * (t.ti + 1) / 2 : (long)t.ti * t.tj;
             int cnt = 0;
             for (int si0 = 0; si0 < t.ti; si0 += pt.sbi)
@@ -377,7 +380,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     // ---- workspace plan: all spin blocks resident or one at a time, k chunk kc and tile edge T under the budget ----------------
     const size_t budget = workspace_budget(c);
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
-    const int tcap = contract_full_max_tile();
+    const int tcap = contract_full_max_tile(), tpref = contract_full_pref_tile();
     int kc = nvec, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
     auto fixed_bytes = [&](int kc_, bool res) {
         size_t f = grid_b * (size_t)kc_ * ((size_t)(res ? sumsrc : maxsrc) + (size_t)maxsrc);
@@ -388,7 +391,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     };
     for (;;) {
         fixed = fixed_bytes(kc, resident);
-        T = std::min(std::min(maxsrc, tcap), c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tcap);
+        T = std::min(maxsrc, c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tpref);
         const int tmin = std::min(maxsrc, 16);
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 4);
         const bool fits = fixed + grid_b * (size_t)T * T <= budget;
@@ -401,7 +404,10 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     }
     if (nblk == 1) resident = true;
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
-    int rc = ensure_arena(c, fixed + grid_b * (size_t)T * T);
+    // width of the off-diagonal tiles: as many row blocks as the budget holds (at most what is right of the first row block)
+    int W = T;
+    while (W < maxsrc - T && fixed + grid_b * (size_t)T * (W + T) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;
+    int rc = ensure_arena(c, fixed + grid_b * (size_t)T * W);
     if (rc) return rc;
     char* p = c->arena;
     auto carve = [&](size_t bytes) { char* q = p; p += (bytes + 255) / 256 * 256; return (double*)q; };
@@ -417,9 +423,9 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     if (rot) { Xr = (cplx*)carve(sizeof(cplx) * (size_t)kc * maxsrc * npwh); Yr = (cplx*)carve(sizeof(cplx) * (size_t)kc * maxsrc * npwh); }
     const size_t o_cap = project_scratch_doubles(c, maxbasis, kc * maxsrc, budget);
     double* O = carve(sizeof(double) * o_cap);
-    double* tau = carve(grid_b * (size_t)T * T);
-    for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src])); if (rc) return rc; }
-    c->last_pair_tile = T; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = kc; c->last_resident = resident ? 1 : 0;
+    double* tau = carve(grid_b * (size_t)T * W);
+    for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src]), W); if (rc) return rc; }
+    c->last_pair_tile = T; c->last_tile_width = W; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = kc; c->last_resident = resident ? 1 : 0;
 
     for (int k0 = 0; k0 < nvec; k0 += kc) {
         const int kcc = std::min(kc, nvec - k0);
@@ -591,6 +597,7 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
             c->dav_block = opt->block; c->dav_precond = opt->precond; c->verbose = opt->verbose;
             c->fused = opt->fft_path == 0;
+            c->tile_width = opt->tile_width;
             if (opt->work_l2_mb > 0) c->work_l2_mb = opt->work_l2_mb;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
             if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");
@@ -808,7 +815,7 @@ int tddft_set_timing(tddft_ctx* c, int enabled) { if (!c) return TDDFT_EINVAL; c
 int tddft_get_stats(const tddft_ctx* c, tddft_stats* out) {
     if (!c || !out) return TDDFT_EINVAL;
     *out = c->stats; out->fft_batch = c->fft_batch; out->fft_path = c->fused ? 0 : 1;
-    out->pair_batch = c->last_pair_batch; out->pair_tile = c->last_pair_tile; out->k_chunk = c->last_kc; out->blocks_resident = c->last_resident;
+    out->pair_batch = c->last_pair_batch; out->pair_tile = c->last_pair_tile; out->tile_width = c->last_tile_width; out->k_chunk = c->last_kc; out->blocks_resident = c->last_resident;
     return TDDFT_OK;
 }
 

@@ -40,13 +40,18 @@ struct ZArgs {
     double sscale;
     const int* slots;      // optional (device, already offset to this launch): function index of packed function q is slots[q]
     // layout of the real function batches src0/src1/dst: function index fbase + (0..nfun-1) inside a batch of ftotal
-    // functions; chunked = 0: [f][nr];  chunked = 1: [nr/32][ftotal][32] (CHUNK consecutive grid points per function)
+    // functions; chunked = 0: [f][nr];  chunked = 1: [nr/CHUNK][ftotal][CHUNK] (CHUNK consecutive grid points per function)
     int chunked; long fbase; long ftotal;
     // fused path only: pruned layout of the work grids (plan.h): column map, live columns, grid stride in `work`
     const int* cmap; int ncols; long wstride;
     int whint;             // L2 policy of the work-grid stream: 1 = evict first, 0 = normal (the launch's work grids fit in L2)
 };
-constexpr int CHUNK = 32;
+// Chunked layout of real-space function batches: [nr/CHUNK][function][CHUNK].  The plane kernels write CHUNK consecutive points
+// of a function as one run and a CTA of the contraction (contract.cu) reads 4 points (32 bytes) of every function.  Measured at
+// config 3 (block apply, S4 + S5 ms): CHUNK 32: 627 + 320; 16: 640 + 322; 8: 655 + 297; 4: 689 + 266 -- what the contraction gains
+// from longer runs of its own the pair-FFT pipeline loses on its stores, the sum stays within 1 %; 32 is kept.
+constexpr int CHUNK_LOG = 5;
+constexpr int CHUNK = 1 << CHUNK_LOG;
 inline long chunked_elems(long nfun, long nr) { return (nr + CHUNK - 1) / CHUNK * CHUNK * nfun; }
 // strided passes along an axis with element stride `stride` over `inner` contiguous elements, `nouter` slabs
 enum SMode { SM_FWD = 0, SM_INV = 1, SM_CONV = 2 /* forward, multiply by ktab, inverse */ };

@@ -14,7 +14,7 @@ struct TileInfo {
     long nslots;               // tau slots of the tile (dense ti*tj, or ti(ti+1)/2 on the diagonal)
 };
 struct PairTiles {
-    int T = 0, nocc = 0;
+    int T = 0, W = 0, nocc = 0;
     std::vector<TileInfo> tiles;
     int2* d_pairs = nullptr;   // pairs in processing order (sub-blocks of sbi x sbj, so a batch touches few orbitals)
     int* d_pslot = nullptr;    // tau slot of each pair of d_pairs
@@ -38,7 +38,7 @@ struct tddft_ctx {
     cudaStream_t stream = nullptr;
     double workspace_gb = 0;
     double work_l2_mb = 48.0;        // launches with smaller work grids keep them under the normal L2 policy
-    int pair_tile = 0, fft_batch = 0;
+    int pair_tile = 0, fft_batch = 0, tile_width = 0;
     int num_sms = 148;
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off
     int dav_max_subspace = 0, dav_max_iter = 0, dav_block = 0, dav_precond = 0, verbose = 0;
@@ -74,7 +74,7 @@ struct tddft_ctx {
     bool overlap_copies = false;     // set only while tddft_apply_liouville_host drives an apply
     // bookkeeping
     tddft_stats stats{};
-    int last_pair_batch = 0, last_pair_tile = 0, last_kc = 0, last_resident = 1;
+    int last_pair_batch = 0, last_pair_tile = 0, last_tile_width = 0, last_kc = 0, last_resident = 1;
     bool timing = false;
     std::vector<StageEvent> events;
     std::string err;
@@ -101,7 +101,7 @@ int hartree(tddft_ctx* c, const double* d0, const double* d1, double scale, int 
 // tau_p = C[A1[x_p] A2[y_p]] for npairs pairs (device lists), written to slot d_slots[p] (or p) of a batch of stot functions
 int pair_potentials_dev(tddft_ctx* c, const double* A1, const double* A2, const int2* d_pairs, const int* d_slots, long npairs,
                         int batch_pairs, double* tau, int chunked, long stot);
-int build_tiles(tddft_ctx* c, int spin, int T);
+int build_tiles(tddft_ctx* c, int spin, int T, int W);
 int orbital_overlap(tddft_ctx* c, int spin, double* S);     // Eq. 32, HOST S [N][N]
 // extensions.cu: ACE construction (Eqs. 28-30) from the occupied orbitals plus n_extra further ones (device [n_extra][npwh])
 int build_ace(tddft_ctx* c, int spin, const double* psi_extra, int n_extra);

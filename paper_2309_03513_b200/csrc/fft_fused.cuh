@@ -108,24 +108,24 @@ struct BLoadPair {
         }
     }
 };
-// Real-function batches (BatchLayout) addressed from one unit: both the chunked layout [nr/32][function][32] and the plain
-// one [function][nr] (which is the chunked formula with a chunk stride of 32 elements) put point idx of function f at
-//   f_off + (idx >> 5) * cstride + (idx & 31),   f_off = f*32 (chunked) or f*nr (plain).
+// Real-function batches (BatchLayout) addressed from one unit: both the chunked layout [nr/CHUNK][function][CHUNK] and the plain
+// one [function][nr] (which is the chunked formula with a chunk stride of CHUNK elements) put point idx of function f at
+//   f_off + (idx / CHUNK) * cstride + (idx % CHUNK),   f_off = f*CHUNK (chunked) or f*nr (plain).
 // A bound functor keeps the byte address of (function, chunk of the plane's first point) and turns a plane offset into
 // one shift, one mask and one 32x32->64 multiply-add.
 struct UnitAddr {
-    unsigned r0;        // (first point of the plane) & 31
+    unsigned r0;        // (first point of the plane) & (CHUNK - 1)
     unsigned cs8;       // chunk stride in bytes
     __device__ __forceinline__ size_t operator()(int off) const {
         const unsigned i = r0 + (unsigned)off;
-        return (size_t)(i >> 5) * cs8 + (size_t)((i & 31u) * 8u);
+        return (size_t)(i >> CHUNK_LOG) * cs8 + (size_t)((i & (unsigned)(CHUNK - 1)) * 8u);
     }
 };
 __device__ __forceinline__ UnitAddr unit_addr(const BatchLayout& lay, long pbase) {
-    return UnitAddr{(unsigned)(pbase & 31), (unsigned)((lay.chunked ? lay.cstride : 32) * 8)};
+    return UnitAddr{(unsigned)(pbase & (CHUNK - 1)), (unsigned)((lay.chunked ? lay.cstride : CHUNK) * 8)};
 }
 __device__ __forceinline__ long fun_base(const BatchLayout& lay, long f, long pbase) {   // element offset of (f, chunk of pbase)
-    return lay.chunked ? (pbase >> 5) * lay.cstride + (lay.fbase + f) * CHUNK : (lay.fbase + f) * lay.nr + (pbase & ~31L);
+    return lay.chunked ? (pbase >> CHUNK_LOG) * lay.cstride + (lay.fbase + f) * CHUNK : (lay.fbase + f) * lay.nr + (pbase & ~(long)(CHUNK - 1));
 }
 struct BLoadPack2 {
     const char *p0, *q0; long d1; UnitAddr ua; bool has_im; double scale;   // p0/q0: function 2b of src0/src1 (q0 may be null); d1: bytes to 2b+1

@@ -30,7 +30,7 @@ struct LoadPair {      // pair p = (x, y): density phi[x] * phi2[y] (both plain 
 struct BatchLayout {     // address of grid point idx of function f inside a batch of real functions (common.h)
     int chunked; long fbase, cstride, nr;
     __device__ __forceinline__ long operator()(long f, long idx) const {
-        return chunked ? (idx >> 5) * cstride + (fbase + f) * CHUNK + (idx & (CHUNK - 1)) : (fbase + f) * nr + idx;
+        return chunked ? (idx >> CHUNK_LOG) * cstride + (fbase + f) * CHUNK + (idx & (CHUNK - 1)) : (fbase + f) * nr + idx;
     }
     __device__ __forceinline__ long next() const { return chunked ? CHUNK : nr; }   // offset from function f to f + 1
 };

@@ -77,7 +77,7 @@ __global__ void drho_kernel(const double* __restrict__ phi, const double* __rest
     double acc[KC];
 #pragma unroll
     for (int q = 0; q < KC; ++q) acc[q] = 0.0;
-    const double* ac = a + (r >> 5) * ((long)nocc * kc * CHUNK) + (r & (CHUNK - 1));
+    const double* ac = a + (r >> CHUNK_LOG) * ((long)nocc * kc * CHUNK) + (r & (CHUNK - 1));
     for (int v = 0; v < nocc; ++v) {
         const double p = phi[(long)v * nr + r];
         const double* av = ac + ((long)v * kc + kk0) * CHUNK;
@@ -185,14 +185,14 @@ __global__ void pattern_reduce_kernel(const double* __restrict__ M, const double
     double acc[KT];
 #pragma unroll
     for (int q = 0; q < KT; ++q) acc[q] = 0.0;
-    const double* tc = tau + (r >> 5) * ((long)nj * nt * CHUNK) + (r & (CHUNK - 1));
+    const double* tc = tau + (r >> CHUNK_LOG) * ((long)nj * nt * CHUNK) + (r & (CHUNK - 1));
     for (int j = 0; j < nj; ++j) {
         const double m = M[(long)j * nr + r];
         const double* tj = tc + ((long)j * nt + t0) * CHUNK;
 #pragma unroll
         for (int q = 0; q < KT; ++q) if (t0 + q < tend) acc[q] = fma(m, tj[q * CHUNK], acc[q]);
     }
-    double* oc = out + (r >> 5) * (ftot * CHUNK) + (r & (CHUNK - 1));
+    double* oc = out + (r >> CHUNK_LOG) * (ftot * CHUNK) + (r & (CHUNK - 1));
 #pragma unroll
     for (int q = 0; q < KT; ++q) if (t0 + q < tend) { double* o = oc + (f0 + (long)q * fstep) * CHUNK; *o = fma(scale, acc[q], *o); }
 }

@@ -30,10 +30,12 @@ cudaError_t launch_out_init(const double* phi, const double* V, const double* vl
                             double* out, cudaStream_t st);
 // S5 (Eq. 6) on batches in the chunked layout [nr/32][function][32] (common.h); ftot = functions in
 // a/out (nocc*kc), stot = slots in the tau tile.
-// Register-resident tiles: one launch does a whole tile with up to contract_full_max_tile() rows (any number of
-// columns); diag: ti == tj, same orbital block, tau packed upper-triangular (one direction, symmetric reads); else dense
-// slots i*tj + j and both directions.  stot = slots in the tau tile.
+// Register-resident tiles (contract.cu): one launch does a whole tile with up to contract_full_max_tile() rows (any number of
+// columns); contract_full_pref_tile() is the edge the default plan uses (the largest one whose kernel keeps registers free for
+// running fragment loads ahead of the DMMAs).  diag: ti == tj, same orbital block, tau packed upper-triangular (one direction,
+// symmetric reads); else dense slots i*tj + j and both directions.
 int contract_full_max_tile();
+int contract_full_pref_tile();
 cudaError_t launch_contract_full(bool diag, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj, int kc,
                                  long ftot, long stot, long nr, double alpha, cudaStream_t st);
 // spin-flip K1e potential V[kk][r] = f[r] * d[kk][r] (Eq. 24); D term alone AX = (kin - eig_v) X (Eq. 3)

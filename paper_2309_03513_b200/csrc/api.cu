@@ -381,7 +381,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     const size_t budget = workspace_budget(c);
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
     const int tcap = contract_full_max_tile(), tpref = contract_full_pref_tile();
-    int kc = nvec, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
+    int kc = nvec, nkchunks = 1, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
     auto fixed_bytes = [&](int kc_, bool res) {
         size_t f = grid_b * (size_t)kc_ * ((size_t)(res ? sumsrc : maxsrc) + (size_t)maxsrc);
         if (hxc) f += grid_b * (size_t)kc_ * (2 * nblk + 1);
@@ -398,9 +398,11 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
         // a small tile costs a(r)/out(r) traffic in S5: before shrinking T below half its cap, give up residency of all blocks
         if (fits && (T >= std::min(maxsrc, tcap / 2) || (!resident || nblk == 1) )) break;
         if (resident && nblk > 1) { resident = false; continue; }
-        if (fits) break;
+        if (fits && (T >= std::min(maxsrc, 48) || kc == 1)) break;      // a tile edge below 48 costs more in S5 than one more chunk costs in S4
         if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
-        kc = (kc + 1) / 2;
+        // tau is recomputed for every chunk of trial vectors: take the fewest chunks that fit (16 vectors: 16, 8, 6, 4, ...)
+        do { ++nkchunks; } while ((nvec + nkchunks - 1) / nkchunks == kc);
+        kc = (nvec + nkchunks - 1) / nkchunks;
     }
     if (nblk == 1) resident = true;
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest

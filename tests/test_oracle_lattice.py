@@ -103,3 +103,16 @@ def test_grid_must_hold_the_sphere():
     psi = [np.zeros((1, len(miller)), dtype=complex)]; psi[0][0, 0] = 1.0
     with pytest.raises(ValueError):
         olv.Problem(cubic, (12, 12, 10), 10.0, 1, psi, [np.array([-0.1])], 0.0)
+
+
+def test_sphere_counts_match_the_survey_table():
+    """tests/golden/gvector_counts.txt: N_pw / N_pwh of the five BASELINE.json configurations."""
+    import os
+    import synthetic_inputs as inputs
+    path = os.path.join(os.path.dirname(__file__), "golden", "gvector_counts.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 5
+    for cid, npw, npwh in rows:
+        cfg = inputs.config(int(cid))
+        miller, _ = lat.enumerate_half_sphere(np.array(cfg["lattice"], dtype=float), cfg["ecut"])
+        assert len(miller) == int(npwh) and 2 * len(miller) - 1 == int(npw)

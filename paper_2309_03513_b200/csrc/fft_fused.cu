@@ -6,13 +6,24 @@
 namespace tddft {
 
 // (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
-#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8) X(96, 100, 360, 1)
-#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12) X(96)
+#define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8) X(96, 100, 360, 1) X(108, 108, 324, 1)
+#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12) X(96) X(108)
 
 // Launch policy, fixed after the round-1 measurements (profiles/r01g_summary.md, r01i_summary.md): persistent grids that walk
 // the units plane-major; L2 prefetch of the CTA's next work-grid plane (inverse kernels) but not of orbital planes (they are
 // shared with the units running now); evict-first L2 policy on the work-grid / tau / a(r) streams.
 constexpr int kStreamHint = 1;
+// launch with programmatic stream serialization (see pdl_wait in fft_fused.cuh)
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, unsigned block, size_t smem, cudaStream_t s, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 template <int NY, int NZ, int NTHR, int MINB, bool INV, bool DB1, bool DB2, class Load, class Store>
 static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
     static_assert(Two<NY>::ok && Two<NZ>::ok, "fused plane kernel needs two-stage plans");
@@ -31,8 +42,7 @@ static cudaError_t plane_launch2(Load ld, Store st, const ZArgs& a, cudaStream_t
     const int nx = (int)(a.npencils / NY), nunits = nx * a.batch;
     const int grid = nunits < resident[dev] ? nunits : resident[dev];
     const int l2pf = std::is_same<Load, LoadWorkC>::value ? 1 : 0;
-    kern<<<grid, NTHR, smem, s>>>(ld, st, nx, nunits, l2pf, a.tw2, a.tw);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3(grid), NTHR, smem, s, ld, st, nx, nunits, l2pf, a.tw2, a.tw);
 }
 template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
 static cudaError_t plane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
@@ -84,10 +94,9 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     }
     dim3 grid(tiles, (unsigned)best_gy);
     constexpr int NT = XCfg<NX>::NTHR;
-    if (mode == SM_FWD) xpass_kernel<NX, SM_FWD><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
-    else if (mode == SM_INV) xpass_kernel<NX, SM_INV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
-    else xpass_kernel<NX, SM_CONV><<<grid, NT, smem, s>>>(a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
-    return cudaGetLastError();
+    if (mode == SM_FWD) return launch_pdl(xpass_kernel<NX, SM_FWD>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    if (mode == SM_INV) return launch_pdl(xpass_kernel<NX, SM_INV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    return launch_pdl(xpass_kernel<NX, SM_CONV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
 }
 
 bool fused_supported(const int* n) {

@@ -28,6 +28,12 @@ template <int N> struct Two {   // two-stage view of Plan<N>
     __host__ __device__ static constexpr int pad(int e) { return PADP ? e + e / PADP : e; }
 };
 
+// Programmatic dependent launch (fft_fused.cu launches these kernels with programmaticStreamSerialization): a kernel lets its
+// successor in the stream start launching at once (its CTAs take the SM slots this kernel's CTAs free, and run their prologue:
+// twiddles, column maps, Coulomb-table values), and waits for its predecessor to complete before it touches any work buffer.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // twiddles of residue i: w[r] = tw[i*r], r = 1..R1-1 (w[0] unused)
 template <int R1> __device__ __forceinline__ void load_twiddles(const cplx* __restrict__ tw, int i, cplx (&w)[R1]) {
     w[0] = make_double2(1.0, 0.0);
@@ -211,6 +217,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
     static_assert(NTHR % R2z == 0 && NTHR % R2y == 0, "a thread's residue must be the same in every round");
     extern __shared__ cplx sm[];
     const int tid = threadIdx.x;
+    pdl_launch_dependents();
     cplx wz[R1z], wy[R1y];
     load_twiddles<R1z>(twz_g, tid % R2z, wz);
     if constexpr (NY == NZ) {
@@ -256,6 +263,7 @@ __global__ void __launch_bounds__(NTHR) __maxnreg__((PlaneRegs<NTHR, MINB>::valu
         }
     }
 
+    pdl_wait();
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int xpl = u / nbatch, b = u - xpl * nbatch;
         BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
@@ -464,6 +472,7 @@ template <int NX> struct XCfg {
 template <int NX, int MODE>
 __global__ void __launch_bounds__(XCfg<NX>::NTHR, XCfg<NX>::MINB) xpass_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
                                                                  const cplx* __restrict__ tw_g, const double* __restrict__ ktab, int hint) {
+    pdl_launch_dependents();
     const unsigned long long pol = l2_policy(hint);
     constexpr int R1 = XCfg<NX>::R1, R2 = XCfg<NX>::R2;
     extern __shared__ cplx sm[];
@@ -475,6 +484,7 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, XCfg<NX>::MINB) xpass_kernel(c
 #pragma unroll
         for (int k = 0; k < R2; ++k) kt[k] = (live && g < R1) ? __ldg(ktab + (long)(g * R2 + k) * inner + col) : 0.0;
     }
+    pdl_wait();
     for (int b = blockIdx.y; b < batch; b += gridDim.y) {
         cplx* gcol = work + (long)b * nr + col;
         if (MODE == SM_FWD || MODE == SM_CONV) {

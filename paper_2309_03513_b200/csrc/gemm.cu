@@ -101,7 +101,7 @@ static cudaError_t nt_pipe_launch(const double* A, long lda, const double* B, lo
 }
 typedef GemmCfg<144, 128, 72, 32, 4> NtBig;     // orbitals x functions: 432 = 3 x 144, 1150 ~ 8 x 144
 typedef GemmCfg<64, 64, 32, 32, 4> NtSmall;     // Davidson Gram matrices (m <= a few hundred, K = 10^7)
-typedef GemmCfg<128, 144, 32, 72, 4> TnBig;
+typedef GemmCfg<128, 72, 32, 72, 4, 2> TnBig;    // two 4-warp CTAs per SM: one epilogue (C read-modify-write) runs behind the other DMMAs
 
 int gemm_nt_tile_count(int M, int N) {
     if (M >= 96 && N >= 96) return ((M + NtBig::BM - 1) / NtBig::BM) * ((N + NtBig::BN - 1) / NtBig::BN);

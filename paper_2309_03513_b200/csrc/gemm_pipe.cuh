@@ -22,8 +22,8 @@ __device__ __forceinline__ void cp16z(void* smem, const void* gmem, int bytes) {
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int BM_, int BN_, int WM_, int WN_, int STAGES_> struct GemmCfg {
-    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, STAGES = STAGES_;
+template <int BM_, int BN_, int WM_, int WN_, int STAGES_, int MINB_ = 1> struct GemmCfg {
+    static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, STAGES = STAGES_, MINB = MINB_;   // MINB: CTAs per SM
     static constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN, NTHR = 32 * WARPS_M * WARPS_N;
     static constexpr int FM = WM / 8, FN = WN / 8;
     // NT: rows K-contiguous, pitch GK + 4;  TN: rows M/N-contiguous, pitch = 4 mod 16
@@ -129,7 +129,7 @@ gemm_nt_pipe_kernel(const double* __restrict__ A, long lda, const double* __rest
 // C[m][n] += cscale * sum_k At[k][m] B[k][n];  C row m at C + (m / cgrp)*cstride_grp + (m % cgrp)*ldc.
 // At rows (ldat) and B rows (ldb) must start 16-byte aligned (ldat, ldb even).
 template <class CFG>
-__global__ void __launch_bounds__(CFG::NTHR, 1)
+__global__ void __launch_bounds__(CFG::NTHR, CFG::MINB)
 gemm_tn_pipe_kernel(const double* __restrict__ At, long ldat, const double* __restrict__ B, long ldb, double* __restrict__ C, long ldc,
                     int cgrp, long cstride_grp, int M, long N, int K, double cscale) {
     constexpr int BM = CFG::BM, BN = CFG::BN, LDM = CFG::LDM, LDN = CFG::LDN, ST = CFG::STAGES, NTHR = CFG::NTHR, FM = CFG::FM, FN = CFG::FN;

@@ -255,6 +255,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=0)
     ap.add_argument("--precond", type=int, default=0)
     ap.add_argument("--verbose", type=int, default=0)
+    ap.add_argument("--probes", action="store_true", help="also run the read-bandwidth probe (fp64_peaks.read_gbs_by_piece_bytes)")
     args = ap.parse_args()
 
     import synthetic_inputs as inputs
@@ -370,6 +371,8 @@ def main():
     if rank == 0:
         dfma, dmma = b.tddft_fp64_peak(ctx)
         fp64 = {"dfma_tflops": dfma, "dmma_tflops": dmma}
+        if args.probes:      # read bandwidth of the contraction's access pattern (32-byte pieces) against whole 256-byte runs
+            fp64["read_gbs_by_piece_bytes"] = {str(pb_): b.tddft_stream_probe(ctx, pb_) for pb_ in (32, 64, 128, 256)}
         if not args.no_coupling and mode == 0:
             b.tddft_apply_coupling(ctx, dX[:1], dAX[:1], 1, 0)      # warm-up
             torch.cuda.synchronize()

@@ -198,6 +198,10 @@ int tddft_exchange_apply(tddft_ctx* ctx, int spin, const double* Y, double* VY, 
 /* FP64 peak probes for the roofline denominators (bench.py): register-resident DFMA and DMMA (mma.sync.m8n8k4.f64) loops on
  * every SM, timed with CUDA events on the context's stream.  Both in TFLOP/s, HOST outputs. */
 int tddft_fp64_peak(tddft_ctx* ctx, double* dfma_tflops, double* dmma_tflops);
+/* Read-bandwidth probe for the access pattern of the exchange contraction (S5): CTAs stream piece_bytes-byte pieces (32, 64, 128 or
+ * 256) at a 256-byte stride, 256/piece_bytes CTAs sharing every 256-byte run, over 8 GB.  GB/s, HOST output; CUDA events on the
+ * context's stream.  32 is what a contraction CTA (4 grid points of a 32-point chunk) does; 256 is a plain streaming read. */
+int tddft_stream_probe(tddft_ctx* ctx, int piece_bytes, double* gbs);
 
 const char* tddft_last_error(const tddft_ctx* ctx); /* ctx may be NULL: error of the last failed tddft_init */
 int tddft_destroy(tddft_ctx* ctx);

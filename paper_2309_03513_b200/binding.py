@@ -20,7 +20,7 @@ EXPORTS = [
     "tddft_workspace_bytes", "tddft_apply_liouville", "tddft_apply_liouville_host", "tddft_davidson",
     "tddft_set_timing", "tddft_get_stats", "tddft_pair_potentials", "tddft_project", "tddft_gram",
     "tddft_orbital_real_space", "tddft_last_error", "tddft_destroy", "tddft_apply_coupling", "tddft_orbital_overlap",
-    "tddft_exchange_apply", "tddft_fp64_peak",
+    "tddft_exchange_apply", "tddft_fp64_peak", "tddft_stream_probe",
 ]
 
 
@@ -256,6 +256,12 @@ def tddft_fp64_peak(ctx):
     a = C.c_double(0.0); b = C.c_double(0.0)
     _check(_lib.tddft_fp64_peak(ctx._h, C.byref(a), C.byref(b)), ctx._h)
     return a.value, b.value
+
+
+def tddft_stream_probe(ctx, piece_bytes):
+    g = C.c_double(0)
+    _check(_lib.tddft_stream_probe(ctx._h, C.c_int(piece_bytes), C.byref(g)), ctx._h)
+    return g.value
 
 
 def tddft_last_error(ctx=None):

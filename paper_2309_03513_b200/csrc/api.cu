@@ -135,7 +135,9 @@ int pair_potentials_dev(tddft_ctx* c, const double* A1, const double* A2, const 
 }
 
 // S1: nfun half-sphere functions -> real space, dst[f][r] = Omega^-1/2 sum_G c_f(G) exp(i G.r)
-int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked) {
+// The nfun functions are functions fbase0 .. fbase0 + nfun - 1 of a destination batch of ftotal functions (ftotal <= 0: nfun).
+int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked, long fbase0, long ftotal) {
+    if (ftotal <= 0) ftotal = nfun;
     const double scale = 1.0 / std::sqrt(c->hp.omega);
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
@@ -143,7 +145,7 @@ int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* 
         TD_CUDA(c, launch_scatter_pack2(X, lay, f0, nfun, nb, c->d_idx_p, c->d_idx_m, c->d_work, work_stride(c, KIND_SPHERE), c->stream));
         TD_RC(leg_x(c, SM_INV, nb, KIND_SPHERE));
         ZArgs z = zpass_args(c, nb, KIND_SPHERE);
-        z.dst = dst; z.nfun = nf; z.sscale = scale; z.chunked = chunked; z.fbase = f0; z.ftotal = nfun;
+        z.dst = dst; z.nfun = nf; z.sscale = scale; z.chunked = chunked; z.fbase = fbase0 + f0; z.ftotal = ftotal;
         TD_RC(leg_inverse_yz(c, z));
         c->stats.kernel_launches += 1;
     }
@@ -151,17 +153,20 @@ int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* 
 }
 
 // S6+S7: real-space functions (chunked batch) -> half sphere, AX = (Omega^1/2/N_r) FFT[src] + (|G|^2/2 - eps_v) X; X = null: no D term
-int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig) {
+// src: functions fbase0 .. fbase0 + nfun - 1 of a chunked batch of ftotal functions (ftotal <= 0: nfun); accumulate (X == null): AX += result
+int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig, long fbase0, long ftotal,
+                     bool accumulate) {
+    if (ftotal <= 0) ftotal = nfun;
     const long nr = c->hp.nr;
     const double scale = std::sqrt(c->hp.omega) / (double)nr;
     for (int f0 = 0; f0 < nfun; f0 += 2 * c->fft_batch) {
         const int nf = std::min(2 * c->fft_batch, nfun - f0);
         const int nb = (nf + 1) / 2;
         ZArgs z = zpass_args(c, nb, KIND_SPHERE);
-        z.src0 = src; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0; z.chunked = 1; z.fbase = f0; z.ftotal = nfun;
+        z.src0 = src; z.src1 = nullptr; z.nfun = nf; z.lscale = 1.0; z.chunked = 1; z.fbase = fbase0 + f0; z.ftotal = ftotal;
         TD_RC(leg_forward_yz(c, ZL_PACK2, z));
         TD_RC(leg_x(c, SM_FWD, nb, KIND_SPHERE));
-        TD_CUDA(c, launch_gather_unpack2(c->d_work, work_stride(c, KIND_SPHERE), c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream));
+        TD_CUDA(c, launch_gather_unpack2(c->d_work, work_stride(c, KIND_SPHERE), c->d_idx_p, c->d_idx_m, f0, nfun, nb, scale, X, AX, lay, c->d_kin, d_eig, c->stream, accumulate));
         c->stats.kernel_launches += 1;
     }
     return TDDFT_OK;
@@ -353,6 +358,171 @@ static int rotate_rows(tddft_ctx* c, int spin, bool back, const double* src, lon
 // ---- one application ------------------------------------------------------------------------------
 struct Block { int src, tgt; long off; };   // occupied spin, target spin, offset (complex) inside a trial vector
 
+// ---- one application, streamed plan -------------------------------------------------------------------------------
+// Used when a(r) and out(r) of a whole spin block do not fit for all trial vectors (configs 4, 5).  The tile loop is outermost:
+// tau of a tile is formed ONCE and the trial vectors are looped inside it, ks at a time; a(r) of the tile's rows and columns is
+// recomputed from X for every tile (S1 on (ti + tj)*ks functions) and the tile's contribution to out goes back to the sphere at
+// once and is ADDED to AX there (S6 in accumulate mode), so no real-space array is longer than a tile edge.  The extra transforms
+// are ~32 (1/ti + 1/tj) per pair FFT (Eq. 6: the pair potentials do not depend on the trial vectors).
+static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const std::vector<Block>& blocks, bool hxc, bool sfk, long L, size_t budget) {
+    const long nr = c->hp.nr, npwh = c->hp.npwh;
+    const int nblk = (int)blocks.size();
+    const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);
+    int maxsrc = 0, maxbasis = 0; bool rot = false;
+    for (auto& b : blocks) {
+        maxsrc = std::max(maxsrc, c->nocc[b.src]);
+        maxbasis = std::max(maxbasis, std::max(c->nocc[b.tgt], c->n_ace[b.tgt]));
+        rot = rot || c->d_U[b.src];
+    }
+    // ---- plan: tile T x W, ks vectors at a time
+    const int tcap = contract_full_max_tile(), tpref = contract_full_pref_tile();
+    int T = std::min(maxsrc, c->pair_tile > 0 ? std::min(c->pair_tile, tcap) : tpref), ks = nvec, nks = 1;
+    size_t fixed = 0;
+    auto fixed_bytes = [&]() {
+        size_t f = 0;
+        if (hxc) f += grid_b * (size_t)nvec * (2 * nblk + 1);
+        if (sfk) f += grid_b * (size_t)nvec * 2;
+        if (rot) f += 2 * sizeof(cplx) * (size_t)nvec * maxsrc * npwh;
+        return f + sizeof(double) * project_scratch_doubles(c, maxbasis, nvec * maxsrc, budget) + 16384;
+    };
+    fixed = fixed_bytes();
+    auto need = [&](int T_, int W_, int ks_) { return fixed + grid_b * ((size_t)T_ * W_ + 2 * (size_t)(T_ + W_) * ks_); };
+    for (;;) {
+        if (need(T, T, ks) <= budget) break;
+        if (ks > 1 && (ks > 8 || T <= 48)) { do { ++nks; } while ((nvec + nks - 1) / nks == ks); ks = (nvec + nks - 1) / nks; continue; }
+        if (T > 16) { T = std::max(16, T - 4); continue; }
+        return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the streamed plan");
+    }
+    { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }
+    int W = T;
+    while (W < maxsrc - T && need(T, W + T, ks) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;
+    int rc = ensure_arena(c, need(T, W, ks));
+    if (rc) return rc;
+    char* p = c->arena;
+    auto carve = [&](size_t bytes) { char* q = p; p += (bytes + 255) / 256 * 256; return (double*)q; };
+    double* A = carve(grid_b * (size_t)(T + W) * ks);
+    double* O_ = carve(grid_b * (size_t)(T + W) * ks);
+    std::vector<double*> drho(nblk, nullptr), V(nblk, nullptr);
+    double* vh = nullptr;
+    if (hxc) { for (int b = 0; b < nblk; ++b) { drho[b] = carve(grid_b * nvec); V[b] = carve(grid_b * nvec); } vh = carve(grid_b * nvec); }
+    if (sfk) { drho[0] = carve(grid_b * nvec); V[0] = carve(grid_b * nvec); }
+    cplx *Xr = nullptr, *Yr = nullptr;
+    if (rot) { Xr = (cplx*)carve(sizeof(cplx) * (size_t)nvec * maxsrc * npwh); Yr = (cplx*)carve(sizeof(cplx) * (size_t)nvec * maxsrc * npwh); }
+    const size_t o_cap = project_scratch_doubles(c, maxbasis, nvec * maxsrc, budget);
+    double* Oproj = carve(sizeof(double) * o_cap);
+    double* tau = carve(grid_b * (size_t)T * W);
+    for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src]), W); if (rc) return rc; }
+    c->last_pair_tile = T; c->last_tile_width = W; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = ks; c->last_resident = 0;
+
+    if (c->overlap_copies) for (int b = 0; b < nblk; ++b) TD_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_x_ready[b], 0));
+    // source of the real-space transforms of block b: X, or the rotated functions of Eq. 31 (one block at a time in Xr)
+    auto source = [&](int b, const cplx** src, long* vlen, long* boff) -> int {
+        const Block& bl = blocks[b];
+        const int no = c->nocc[bl.src];
+        if (!c->d_U[bl.src]) { *src = X; *vlen = L; *boff = bl.off; return TDDFT_OK; }
+        StageTimer t(c, ST_S7X);
+        TD_RC(rotate_rows(c, bl.src, false, (const double*)(X + bl.off), 2 * L, (double*)Xr, 2L * no * npwh, nvec, false));
+        *src = Xr; *vlen = (long)no * npwh; *boff = 0;
+        return TDDFT_OK;
+    };
+    // ---- S2 / S3 for all trial vectors: drho by row groups, then the potentials
+    if (hxc || sfk) {
+        for (int b = 0; b < nblk; ++b) {
+            const Block& bl = blocks[b];
+            const int no = c->nocc[bl.src];
+            TD_RC(ensure_phi(c, bl.src));
+            const cplx* src; long vlen, boff;
+            TD_RC(source(b, &src, &vlen, &boff));
+            for (int g0 = 0; g0 < no; g0 += T + W) {
+                const int tg = std::min(T + W, no - g0);
+                for (int k0 = 0; k0 < nvec; k0 += ks) {
+                    const int kcc = std::min(ks, nvec - k0);
+                    { StageTimer t(c, ST_S1);
+                      TD_RC(to_real_space(c, src, FunLayout{vlen, boff + (long)g0 * npwh, npwh, kcc, k0}, tg * kcc, A, 1)); }
+                    StageTimer t(c, ST_S23);
+                    TD_CUDA(c, launch_drho(c->d_phi[bl.src] + (long)g0 * nr, A, tg, kcc, nr, drho[b] + (long)k0 * nr, c->stream, g0 > 0));
+                    c->stats.kernel_launches += (kcc + 3) / 4;
+                }
+            }
+        }
+        StageTimer t(c, ST_S23);
+        if (hxc && c->nspin == 2) {
+            rc = hartree(c, drho[0], drho[1], 1.0, nvec, vh); if (rc) return rc;
+            TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[0], drho[0], c->d_fxc[1], drho[1], nvec, nr, V[0], c->stream));
+            TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[1], drho[0], c->d_fxc[2], drho[1], nvec, nr, V[1], c->stream));
+            c->stats.kernel_launches += 2;
+        } else if (hxc) {
+            rc = hartree(c, drho[0], nullptr, 2.0, nvec, vh); if (rc) return rc;
+            TD_CUDA(c, launch_hxc_potential(vh, c->d_fxc[0], drho[0], c->d_fxc[1], drho[0], nvec, nr, V[0], c->stream));
+            c->stats.kernel_launches += 1;
+        } else {
+            TD_CUDA(c, launch_scale_potential(c->d_fsf, drho[0], nvec, nr, V[0], c->stream)); c->stats.kernel_launches += 1;
+        }
+    }
+    for (int b = 0; b < nblk; ++b) {
+        const Block& bl = blocks[b];
+        const int no = c->nocc[bl.src];
+        TD_RC(ensure_phi(c, bl.src));
+        const double* phi = c->d_phi[bl.src];
+        const cplx* src; long vlen, boff;
+        TD_RC(source(b, &src, &vlen, &boff));
+        const bool rotb = c->d_U[bl.src] != nullptr;
+        // destination of the grid part: AX (started from the D term, Eq. 3) or, with the rotation of Eq. 31, Yr (started from zero)
+        cplx* dst = rotb ? Yr : AX;
+        const long dvlen = rotb ? (long)no * npwh : L, dboff = rotb ? 0 : bl.off;
+        FunLayout lay_full{L, bl.off, npwh, nvec, 0};
+        if (rotb) TD_CUDA(c, cudaMemsetAsync(Yr, 0, sizeof(cplx) * (size_t)nvec * no * npwh, c->stream));
+        else { StageTimer t(c, ST_S6); TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1; }
+        const bool has_init = hxc || sfk || c->vloc[bl.tgt];
+        const PairTiles& pt = c->tiles[bl.src];
+        for (const TileInfo& t : pt.tiles) {
+            const bool exch = c->alpha != 0.0 && t.npairs > 0;
+            if (!exch && !(t.diag && has_init)) continue;
+            if (exch) {
+                StageTimer tm(c, ST_S4);
+                if (t.partial) TD_CUDA(c, cudaMemsetAsync(tau, 0, grid_b * (size_t)t.nslots, c->stream));
+                rc = pair_potentials_dev(c, phi, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1, t.nslots); if (rc) return rc;
+            }
+            for (int k0 = 0; k0 < nvec; k0 += ks) {
+                const int kcc = std::min(ks, nvec - k0);
+                const int nI = t.ti * kcc, nJ = t.diag ? 0 : t.tj * kcc;
+                const long ftot = nI + nJ;
+                const FunLayout layI{vlen, boff + (long)t.i0 * npwh, npwh, kcc, k0}, layJ{vlen, boff + (long)t.j0 * npwh, npwh, kcc, k0};
+                { StageTimer tm(c, ST_S1);
+                  TD_RC(to_real_space(c, src, layI, nI, A, 1, 0, ftot));
+                  if (nJ) TD_RC(to_real_space(c, src, layJ, nJ, A, 1, nI, ftot)); }
+                { StageTimer tm(c, ST_S5);
+                  if (t.diag) { TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] + (long)k0 * nr : nullptr, c->vloc[bl.tgt], A, t.ti, kcc, nr, O_, c->stream, ftot)); c->stats.kernel_launches += 1; }
+                  else TD_CUDA(c, cudaMemsetAsync(O_, 0, grid_b * (size_t)ftot, c->stream));
+                  if (exch) {
+                      TD_CUDA(c, launch_contract_full(t.diag, O_, A, tau, 0, t.ti, t.diag ? 0 : t.ti, t.tj, kcc, ftot, t.nslots, nr, c->alpha, c->stream));
+                      c->stats.kernel_launches += (kcc + 15) / 16;
+                  } }
+                StageTimer tm(c, ST_S6);
+                const FunLayout dI{dvlen, dboff + (long)t.i0 * npwh, npwh, kcc, k0}, dJ{dvlen, dboff + (long)t.j0 * npwh, npwh, kcc, k0};
+                TD_RC(to_sphere_plus_d(c, O_, nI, nullptr, dst, dI, nullptr, 0, ftot, true));
+                if (nJ) TD_RC(to_sphere_plus_d(c, O_, nJ, nullptr, dst, dJ, nullptr, nI, ftot, true));
+            }
+        }
+        if (rotb) {       // Eq. 31: rotate the grid part back and add D
+            StageTimer t(c, ST_S7X);
+            TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1;
+            TD_RC(rotate_rows(c, bl.src, true, (const double*)Yr, 2L * no * npwh, (double*)(AX + bl.off), 2 * L, nvec, true));
+        }
+        if (c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {
+            StageTimer t(c, ST_S7X);
+            rc = lowrank_rows(c, (const double*)c->d_xi[bl.tgt], c->n_ace[bl.tgt], (const double*)(X + bl.off), (double*)(AX + bl.off), nvec * no, no, 2 * L,
+                              -c->alpha, Oproj, o_cap);
+            if (rc) return rc;
+        }
+        { StageTimer t(c, ST_S8);
+          rc = project_rows(c, bl.tgt, (double*)(AX + bl.off), nvec * no, no, 2 * L, Oproj, o_cap); if (rc) return rc; }
+        if (c->overlap_copies) TD_CUDA(c, cudaEventRecord(c->ev_ax_done[b], c->stream));
+    }
+    collect_timing(c);
+    return TDDFT_OK;
+}
+
 int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, int mode) {
     if (!c) return TDDFT_EINVAL;
     if (!Xd || !AXd || nvec < 1) return set_err(c, TDDFT_EINVAL, "apply: null buffer or nvec < 1");
@@ -381,7 +551,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     const size_t budget = workspace_budget(c);
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);   // one real grid, padded to whole chunks
     const int tcap = contract_full_max_tile(), tpref = contract_full_pref_tile();
-    int kc = nvec, nkchunks = 1, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
+    int kc = nvec, T = 0; bool resident = !c->phi_shared; size_t fixed = 0;
     auto fixed_bytes = [&](int kc_, bool res) {
         size_t f = grid_b * (size_t)kc_ * ((size_t)(res ? sumsrc : maxsrc) + (size_t)maxsrc);
         if (hxc) f += grid_b * (size_t)kc_ * (2 * nblk + 1);
@@ -396,14 +566,14 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 4);
         const bool fits = fixed + grid_b * (size_t)T * T <= budget;
         // a small tile costs a(r)/out(r) traffic in S5: before shrinking T below half its cap, give up residency of all blocks
-        if (fits && (T >= std::min(maxsrc, tcap / 2) || (!resident || nblk == 1) )) break;
+        if (fits && T >= std::min(maxsrc, tcap / 2)) break;
         if (resident && nblk > 1) { resident = false; continue; }
-        if (fits && (T >= std::min(maxsrc, 48) || kc == 1)) break;      // a tile edge below 48 costs more in S5 than one more chunk costs in S4
-        if (kc == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for a single trial vector");
-        // tau is recomputed for every chunk of trial vectors: take the fewest chunks that fit (16 vectors: 16, 8, 6, 4, ...)
-        do { ++nkchunks; } while ((nvec + nkchunks - 1) / nkchunks == kc);
-        kc = (nvec + nkchunks - 1) / nkchunks;
+        if (fits && T >= std::min(maxsrc, 48)) break;
+        // a(r) / out(r) of a whole spin block do not fit for all trial vectors: tile loop outermost, tau formed once (apply_streamed)
+        kc = 0;
+        break;
     }
+    if (kc < nvec) return apply_streamed(c, X, AX, nvec, blocks, hxc, sfk, L, budget);      // the vectors do not fit together: tile loop outermost
     if (nblk == 1) resident = true;
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
     // width of the off-diagonal tiles: as many row blocks as the budget holds (at most what is right of the first row block)

@@ -95,8 +95,9 @@ int ensure_arena(tddft_ctx* c, size_t bytes);
 int ensure_phi(tddft_ctx* c, int spin);      // makes d_phi[spin] hold that spin's orbitals (phi_shared mode refills)
 size_t workspace_budget(const tddft_ctx* c);
 // real space <-> sphere on batches of functions (api.cu)
-int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked);
-int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig);
+int to_real_space(tddft_ctx* c, const cplx* X, FunLayout lay, int nfun, double* dst, int chunked, long fbase0 = 0, long ftotal = 0);
+int to_sphere_plus_d(tddft_ctx* c, const double* src, int nfun, const cplx* X, cplx* AX, FunLayout lay, const double* d_eig, long fbase0 = 0,
+                     long ftotal = 0, bool accumulate = false);
 int hartree(tddft_ctx* c, const double* d0, const double* d1, double scale, int kc, double* vh);
 // tau_p = C[A1[x_p] A2[y_p]] for npairs pairs (device lists), written to slot d_slots[p] (or p) of a batch of stot functions
 int pair_potentials_dev(tddft_ctx* c, const double* A1, const double* A2, const int2* d_pairs, const int* d_slots, long npairs,

@@ -124,6 +124,47 @@ __global__ void __launch_bounds__(256) dmma_probe_kernel(double* out, int iters)
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+
+// Read-bandwidth probe for the access pattern of the contraction (contract.cu): every CTA streams PIECE-byte pieces at a 256-byte
+// stride (256/PIECE CTAs share each 256-byte run, as the CTAs of one chunk do) through a three-deep cp.async ring.
+template <int PIECE>
+__global__ void __launch_bounds__(128) stream_probe_kernel(const char* __restrict__ src, long rows_per_chunk, int shar, double* __restrict__ out) {
+    extern __shared__ char psm[];
+    const unsigned s0 = (unsigned)__cvta_generic_to_shared(psm);
+    const long chunk = blockIdx.x / shar; const int sub = blockIdx.x % shar;
+    const char* base = src + chunk * rows_per_chunk * 256 + sub * PIECE;
+    constexpr int TPR = PIECE / 16, RPP = 128 / TPR, ROWS = 32768 / PIECE;
+    const int tr = threadIdx.x / TPR, tp = threadIdx.x % TPR;
+    int stage = 0;
+    for (long r0 = 0; r0 < rows_per_chunk; r0 += ROWS, ++stage) {
+        const unsigned sb = s0 + (stage % 3) * 32768;
+        for (int r = tr; r < ROWS && r0 + r < rows_per_chunk; r += RPP)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sb + r * PIECE + tp * 16), "l"(base + (r0 + r) * 256 + tp * 16) : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 2;" ::: "memory");
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) out[blockIdx.x & 1023] = ((const double*)psm)[0];
+}
+template <int PIECE>
+cudaError_t stream_probe_run(const char* buf, size_t bytes, double* out, cudaStream_t st, double* gbs) {
+    const int shar = 256 / PIECE;
+    const long rows = 110L * 110L, nchunks = (long)(bytes / (size_t)(rows * 256));
+    cudaError_t e = cudaFuncSetAttribute(stream_probe_kernel<PIECE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 98304);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    stream_probe_kernel<PIECE><<<(unsigned)(nchunks * shar), 128, 98304, st>>>(buf, rows, shar, out);
+    cudaEventRecord(e0, st);
+    stream_probe_kernel<PIECE><<<(unsigned)(nchunks * shar), 128, 98304, st>>>(buf, rows, shar, out);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *gbs = (double)nchunks * rows * 256.0 / (ms * 1e6);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 }  // namespace
 
 namespace tddft {
@@ -262,6 +303,24 @@ int tddft_fp64_peak(tddft_ctx* c, double* dfma_tflops, double* dmma_tflops) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
     if (e != cudaSuccess) return set_err(c, TDDFT_ECUDA, cudaGetErrorString(e));
     *dfma_tflops = best[0]; *dmma_tflops = best[1];
+    return TDDFT_OK;
+}
+
+int tddft_stream_probe(tddft_ctx* c, int piece_bytes, double* gbs) {
+    if (!c || !gbs || (piece_bytes != 32 && piece_bytes != 64 && piece_bytes != 128 && piece_bytes != 256)) return TDDFT_EINVAL;
+    TD_CUDA(c, cudaSetDevice(c->device));
+    const size_t bytes = (size_t)8 << 30;                       // well beyond the 126 MB L2
+    char* buf = nullptr; bool own = false;
+    if (c->arena_bytes >= bytes + 8192) buf = c->arena + 8192;
+    else { if (cudaMalloc((void**)&buf, bytes) != cudaSuccess) { cudaGetLastError(); return set_err(c, TDDFT_ENOMEM, "stream probe: allocation failed"); } own = true; cudaMemsetAsync(buf, 0, bytes, c->stream); }
+    double* out = nullptr;
+    if (cudaMalloc((void**)&out, 8192) != cudaSuccess) { cudaGetLastError(); if (own) cudaFree(buf); return set_err(c, TDDFT_ENOMEM, "stream probe: allocation failed"); }
+    cudaError_t e = piece_bytes == 32 ? stream_probe_run<32>(buf, bytes, out, c->stream, gbs)
+                  : piece_bytes == 64 ? stream_probe_run<64>(buf, bytes, out, c->stream, gbs)
+                  : piece_bytes == 128 ? stream_probe_run<128>(buf, bytes, out, c->stream, gbs)
+                                       : stream_probe_run<256>(buf, bytes, out, c->stream, gbs);
+    cudaFree(out); if (own) cudaFree(buf);
+    if (e != cudaSuccess) return set_err(c, TDDFT_ECUDA, std::string("stream probe: ") + cudaGetErrorString(e));
     return TDDFT_OK;
 }
 

@@ -33,7 +33,7 @@ cudaError_t launch_scatter_pack2(const cplx* X, FunLayout lay, int f0, int nfun,
 __global__ void gather_unpack2_kernel(const cplx* __restrict__ work, long nr, const int* __restrict__ idx_p,
                                       const int* __restrict__ idx_m, int f0, int nfun, double scale,
                                       const cplx* __restrict__ X, cplx* __restrict__ AX, FunLayout lay,
-                                      const double* __restrict__ kin, const double* __restrict__ eig) {
+                                      const double* __restrict__ kin, const double* __restrict__ eig, int accumulate) {
     const int b = blockIdx.y;
     const int fa = f0 + 2 * b, fb = fa + 1;
     const int va = fa / lay.kc, vb = fb / lay.kc;
@@ -45,9 +45,12 @@ __global__ void gather_unpack2_kernel(const cplx* __restrict__ work, long nr, co
     for (long g = blockIdx.x * (long)blockDim.x + threadIdx.x; g < lay.npwh; g += (long)gridDim.x * blockDim.x) {
         const cplx zp = w[idx_p[g]], zm = w[idx_m[g]];
         // c_A = (Z(G) + conj Z(-G))/2,  c_B = (Z(G) - conj Z(-G))/(2i)
-        if (!X) {      // plain transform to the sphere, no D term
-            AX[oa + g] = make_double2(0.5 * scale * (zp.x + zm.x), 0.5 * scale * (zp.y - zm.y));
-            if (hb) AX[ob + g] = make_double2(0.5 * scale * (zp.y + zm.y), -0.5 * scale * (zp.x - zm.x));
+        if (!X) {      // plain transform to the sphere, no D term (optionally added to what AX holds)
+            cplx ya = make_double2(0.5 * scale * (zp.x + zm.x), 0.5 * scale * (zp.y - zm.y));
+            cplx yb = make_double2(0.5 * scale * (zp.y + zm.y), -0.5 * scale * (zp.x - zm.x));
+            if (accumulate) { const cplx pa = AX[oa + g]; ya.x += pa.x; ya.y += pa.y; if (hb) { const cplx pb = AX[ob + g]; yb.x += pb.x; yb.y += pb.y; } }
+            AX[oa + g] = ya;
+            if (hb) AX[ob + g] = yb;
             continue;
         }
         const double k = kin[g];
@@ -61,9 +64,9 @@ __global__ void gather_unpack2_kernel(const cplx* __restrict__ work, long nr, co
 }
 cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, const int* idx_m, int f0, int nfun, int batch,
                                   double scale, const cplx* X, cplx* AX, FunLayout lay, const double* kin, const double* eig,
-                                  cudaStream_t st) {
+                                  cudaStream_t st, bool accumulate) {
     dim3 grid((unsigned)((lay.npwh + 255) / 256), (unsigned)batch);
-    gather_unpack2_kernel<<<grid, 256, 0, st>>>(work, nr, idx_p, idx_m, f0, nfun, scale, X, AX, lay, kin, eig);
+    gather_unpack2_kernel<<<grid, 256, 0, st>>>(work, nr, idx_p, idx_m, f0, nfun, scale, X, AX, lay, kin, eig, accumulate ? 1 : 0);
     return cudaGetLastError();
 }
 
@@ -71,7 +74,7 @@ cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, c
 // a is in the chunked layout [nr/32][nocc*kc][32] (common.h); phi and drho are plain [.][nr]
 template <int KC>
 __global__ void drho_kernel(const double* __restrict__ phi, const double* __restrict__ a, int nocc, int kc, int kk0, long nr,
-                            double* __restrict__ drho) {
+                            double* __restrict__ drho, int accumulate) {
     const long r = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (r >= nr) return;
     double acc[KC];
@@ -85,11 +88,11 @@ __global__ void drho_kernel(const double* __restrict__ phi, const double* __rest
         for (int q = 0; q < KC; ++q) if (kk0 + q < kc) acc[q] = fma(p, av[q * CHUNK], acc[q]);
     }
 #pragma unroll
-    for (int q = 0; q < KC; ++q) if (kk0 + q < kc) drho[(long)(kk0 + q) * nr + r] = acc[q];
+    for (int q = 0; q < KC; ++q) if (kk0 + q < kc) { double* d = drho + (long)(kk0 + q) * nr + r; *d = accumulate ? *d + acc[q] : acc[q]; }
 }
-cudaError_t launch_drho(const double* phi, const double* a, int nocc, int kc, long nr, double* drho, cudaStream_t st) {
+cudaError_t launch_drho(const double* phi, const double* a, int nocc, int kc, long nr, double* drho, cudaStream_t st, bool accumulate) {
     const unsigned nb = (unsigned)((nr + 127) / 128);
-    for (int kk0 = 0; kk0 < kc; kk0 += 4) drho_kernel<4><<<nb, 128, 0, st>>>(phi, a, nocc, kc, kk0, nr, drho);
+    for (int kk0 = 0; kk0 < kc; kk0 += 4) drho_kernel<4><<<nb, 128, 0, st>>>(phi, a, nocc, kc, kk0, nr, drho, accumulate ? 1 : 0);
     return cudaGetLastError();
 }
 
@@ -111,12 +114,12 @@ cudaError_t launch_hxc_potential(const double* vh, const double* f0, const doubl
 
 // One CTA = one chunk of 32 grid points, all functions: the chunk's nocc*kc rows of 256 bytes are one contiguous run of `out`.
 __global__ void out_init_kernel(const double* __restrict__ phi, const double* __restrict__ V, const double* __restrict__ vloc,
-                                const double* __restrict__ a, int nocc, int kc, long nr, double* __restrict__ out) {
+                                const double* __restrict__ a, int nocc, int kc, long nr, double* __restrict__ out, long ftot) {
     const long chunk = blockIdx.x;
     const int lane = threadIdx.x & (CHUNK - 1), sub = threadIdx.x / CHUNK, nsub = blockDim.x / CHUNK;
     const long r = chunk * CHUNK + lane;
     const bool live = r < nr;
-    const long base = chunk * ((long)nocc * kc * CHUNK) + lane;
+    const long base = chunk * (ftot * CHUNK) + lane;
     const double vl = (vloc && live) ? vloc[r] : 0.0;
     for (int v = sub; v < nocc; v += nsub) {
         const double p = (V && live) ? phi[(long)v * nr + r] : 0.0;
@@ -132,10 +135,11 @@ __global__ void out_init_kernel(const double* __restrict__ phi, const double* __
     }
 }
 cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
-                            double* out, cudaStream_t st) {
+                            double* out, cudaStream_t st, long ftot) {
     const long nchunks = (nr + CHUNK - 1) / CHUNK;
-    if (!V && !vloc) return cudaMemsetAsync(out, 0, sizeof(double) * nchunks * CHUNK * nocc * kc, st);
-    out_init_kernel<<<(unsigned)nchunks, 256, 0, st>>>(phi, V, vloc, a, nocc, kc, nr, out);
+    if (ftot <= 0) ftot = (long)nocc * kc;
+    if (!V && !vloc && ftot == (long)nocc * kc) return cudaMemsetAsync(out, 0, sizeof(double) * nchunks * CHUNK * nocc * kc, st);
+    out_init_kernel<<<(unsigned)nchunks, 256, 0, st>>>(phi, V, vloc, a, nocc, kc, nr, out, ftot);
     return cudaGetLastError();
 }
 

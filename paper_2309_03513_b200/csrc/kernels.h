@@ -17,17 +17,18 @@ cudaError_t launch_scatter_pack2(const cplx* X, FunLayout lay, int f0, int nfun,
 // S6+S7: work grids -> sphere with scale, plus (kin[g] - eig[v]) * x(g)  (Eq. 3); X = null: no D term
 cudaError_t launch_gather_unpack2(const cplx* work, long nr, const int* idx_p, const int* idx_m, int f0, int nfun, int batch,
                                   double scale, const cplx* X, cplx* AX, FunLayout lay, const double* kin, const double* eig,
-                                  cudaStream_t st);
+                                  cudaStream_t st, bool accumulate = false /* X == null only: AX += result */);
 // plain sphere -> grid for one function per complex grid pair is not needed; orbitals use scatter_pack2 too.
 
 // S2: drho[kk][r] = sum_v phi[v][r] * a[v*kc+kk][r]   (inner sum of Eq. 4)
-cudaError_t launch_drho(const double* phi, const double* a, int nocc, int kc, long nr, double* drho, cudaStream_t st);
+cudaError_t launch_drho(const double* phi, const double* a, int nocc, int kc, long nr, double* drho, cudaStream_t st, bool accumulate = false);
 // S3 pointwise: V_s[kk][r] = vh[kk][r] + f_s0[r]*drho0[kk][r] + f_s1[r]*drho1[kk][r]  (drho1/f_s1 may be null)
 cudaError_t launch_hxc_potential(const double* vh, const double* f0, const double* drho0, const double* f1, const double* drho1,
                                  int kc, long nr, double* V, cudaStream_t st);
 // S5 start value: out[f][r] = phi[v][r]*V[kk][r] (if V) + vloc[r]*a[f][r] (if vloc), f = v*kc+kk
+// ftot = functions per chunk of a/out when the nocc*kc functions are the first part of a larger batch (<= 0: nocc*kc)
 cudaError_t launch_out_init(const double* phi, const double* V, const double* vloc, const double* a, int nocc, int kc, long nr,
-                            double* out, cudaStream_t st);
+                            double* out, cudaStream_t st, long ftot = 0);
 // S5 (Eq. 6) on batches in the chunked layout [nr/32][function][32] (common.h); ftot = functions in
 // a/out (nocc*kc), stot = slots in the tau tile.
 // Register-resident tiles (contract.cu): one launch does a whole tile with up to contract_full_max_tile() rows (any number of

@@ -206,3 +206,33 @@ def test_coupling_closed_shell_and_k_chunks():
         b.tddft_apply_coupling(cc.ctx(), dX, dB, 3, 0)
         torch.cuda.synchronize()
         assert rel_fro(dB.cpu().numpy(), ref) < TOL
+
+
+# ---- the 8(f) rows under the streamed plan (api.cu: apply_streamed: tile loop outermost, contributions added in the sphere) ------
+def test_streamed_plan_rotation_truncation_sf_kernel_and_ace():
+    import torch
+    from paper_2309_03513_b200 import binding as b
+    cap = dict(workspace_gb=0.0025, pair_tile=4)
+    rng = np.random.default_rng(16)
+    U = [inputs.random_orthogonal(rng, 6), inputs.random_orthogonal(rng, 4)]
+    mask = [_random_mask(rng, 6, 0.6), _random_mask(rng, 4, 0.6)]
+    trunc = Case(TRI, (12, 18, 20), 6.0, 2, (6, 4), 0.3, seed=352, vloc=True, oracle_opts=dict(wannier_u=U, pair_mask=mask),
+                 wannier_u_up=U[0], wannier_u_dn=U[1], pair_list_up=_mask_to_list(mask[0]), pair_list_dn=_mask_to_list(mask[1]), **cap)
+    for mode in (0, 2):
+        X = trunc.trial(4, mode)
+        got = trunc.gpu_apply(X, mode)
+        assert mode != 0 or b.tddft_get_stats(trunc.ctx())["blocks_resident"] == 0
+        assert rel_fro(got, trunc.oracle.apply(X, mode)) < TOL
+    sf = Case(TRI, (12, 18, 20), 6.0, 2, (5, 3), 0.3, seed=353, oracle_opts=dict(sf_xc_kernel=True, sf_cut=1e-3), sf_xc_kernel=1, sf_cut=1e-3, workspace_gb=0.0015, pair_tile=4)
+    X = sf.trial(4, 1)
+    got = sf.gpu_apply(X, 1)
+    assert b.tddft_get_stats(sf.ctx())["blocks_resident"] == 0
+    assert rel_fro(got, sf.oracle.apply(X, 1)) < TOL
+    case0, extra = _ace_case()
+    d_extra = [torch.from_numpy(e).cuda() for e in extra]
+    xis = [oace.build(case0.oracle, s, extra[s]) for s in range(2)]
+    ca, _ = _ace_case(oracle_opts=dict(ace=xis), ace=1, psi_ace_up=d_extra[0], psi_ace_dn=d_extra[1], workspace_gb=0.002, pair_tile=4)
+    X = ca.trial(4, 0)
+    got = ca.gpu_apply(X, 0)
+    assert b.tddft_get_stats(ca.ctx())["blocks_resident"] == 0
+    assert rel_fro(got, ca.oracle.apply(X, 0)) < 1e-9

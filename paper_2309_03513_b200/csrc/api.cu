@@ -390,7 +390,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
     for (;;) {
         if (need(T, T, ks) <= budget) break;
         if (ks > 1 && (ks > 8 || T <= 48)) { do { ++nks; } while ((nvec + nks - 1) / nks == ks); ks = (nvec + nks - 1) / nks; continue; }
-        if (T > 16) { T = std::max(16, T - 4); continue; }
+        if (T > 2) { T = std::max(2, T - (T > 16 ? 4 : 1)); continue; }
         return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the streamed plan");
     }
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }

@@ -74,7 +74,8 @@ typedef struct {
   const double* x0;         /* device, n_x0 start vectors in the mode's layout, or NULL: library draws its own */
   int n_x0;
   unsigned long long seed;  /* seed of the library's own start vectors */
-  int fft_path;             /* 0 = fused plane/x kernels when the grid shape has them (default), 1 = general pass kernels only */
+  int fft_path;             /* 0 = fused plane/x kernels when the grid shape has them (default), 1 = general pass kernels only,
+                             * 2 = fused, with the two-CTA cluster plane kernel wherever the (y,z) plane shape has one */
   int block;                /* Davidson: most correction vectors appended per iteration; <= 0: nroots */
   int precond;              /* Davidson preconditioner: 0 = projector-aware (reading A11b, default), 1 = diagonal */
   int verbose;              /* 1: tddft_davidson prints one line per iteration on stderr */

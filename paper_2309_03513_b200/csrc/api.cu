@@ -87,7 +87,7 @@ static ZArgs zpass_args(const tddft_ctx* c, int batch, int kind) {
     ZArgs a{}; a.n = n[2]; a.npencils = (long)n[0] * n[1]; a.nr = c->hp.nr; a.batch = batch; a.tw = c->d_tw[2]; a.tw2 = c->d_tw[1]; a.work = c->d_work;
     a.lscale = 1.0; a.sscale = 1.0;
     a.cmap = c->d_cmap[kind]; a.ncols = c->hp.ncols[kind]; a.wstride = work_stride(c, kind);
-    a.whint = work_hint(c, batch, kind);
+    a.whint = work_hint(c, batch, kind); a.cluster = c->prefer_cluster;
     return a;
 }
 
@@ -768,7 +768,8 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->dav_max_subspace = opt->max_subspace; c->dav_max_iter = opt->max_iter; c->dav_tol = opt->tol;
             c->dav_x0 = opt->x0; c->dav_nx0 = opt->n_x0; c->seed = opt->seed;
             c->dav_block = opt->block; c->dav_precond = opt->precond; c->verbose = opt->verbose;
-            c->fused = opt->fft_path == 0;
+            c->fused = opt->fft_path == 0 || opt->fft_path == 2;
+            c->prefer_cluster = opt->fft_path == 2 ? 1 : 0;
             c->tile_width = opt->tile_width;
             if (opt->work_l2_mb > 0) c->work_l2_mb = opt->work_l2_mb;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;

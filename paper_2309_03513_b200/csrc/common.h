@@ -45,6 +45,7 @@ struct ZArgs {
     // fused path only: pruned layout of the work grids (plan.h): column map, live columns, grid stride in `work`
     const int* cmap; int ncols; long wstride;
     int whint;             // L2 policy of the work-grid stream: 1 = evict first, 0 = normal (the launch's work grids fit in L2)
+    int cluster;           // prefer the two-CTA cluster plane kernel (fft_cluster.cuh) where the shape has both variants
 };
 // Chunked layout of real-space function batches: [nr/CHUNK][function][CHUNK].  The plane kernels write CHUNK consecutive points
 // of a function as one run and a CTA of the contraction (contract.cu) reads 4 points (32 bytes) of every function.  Measured at

@@ -40,6 +40,7 @@ struct tddft_ctx {
     double work_l2_mb = 48.0;        // launches with smaller work grids keep them under the normal L2 policy
     int pair_tile = 0, fft_batch = 0, tile_width = 0;
     int num_sms = 148;
+    int prefer_cluster = 0;          // fft_path = 2: two-CTA cluster plane kernels where a shape has both variants
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off
     int dav_max_subspace = 0, dav_max_iter = 0, dav_block = 0, dav_precond = 0, verbose = 0;
     double dav_tol = 0; const double* dav_x0 = nullptr; int dav_nx0 = 0;

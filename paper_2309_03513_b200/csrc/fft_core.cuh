@@ -157,7 +157,7 @@ TD_PLAN(20, 5, 4, 1)   TD_PLAN(24, 6, 4, 1)   TD_PLAN(25, 5, 5, 1)   TD_PLAN(27,
 TD_PLAN(32, 8, 4, 1)   TD_PLAN(36, 6, 6, 1)   TD_PLAN(40, 5, 8, 1)   TD_PLAN(45, 5, 9, 1)   TD_PLAN(48, 6, 8, 1)
 TD_PLAN(50, 5, 10, 1)  TD_PLAN(54, 9, 6, 1)   TD_PLAN(60, 10, 6, 1)  TD_PLAN(64, 8, 8, 1)   TD_PLAN(72, 9, 8, 1)
 TD_PLAN(75, 5, 5, 3)   TD_PLAN(80, 10, 8, 1)  TD_PLAN(81, 9, 9, 1)   TD_PLAN(90, 9, 10, 1)  TD_PLAN(96, 12, 8, 1)
-TD_PLAN(100, 10, 10, 1) TD_PLAN(108, 12, 9, 1) TD_PLAN(120, 5, 6, 4)  TD_PLAN(125, 5, 5, 5)  TD_PLAN(128, 8, 4, 4)
+TD_PLAN(100, 10, 10, 1) TD_PLAN(108, 12, 9, 1) TD_PLAN(120, 5, 6, 4)  TD_PLAN(125, 5, 5, 5)  TD_PLAN(128, 16, 8, 1)
 TD_PLAN(144, 9, 4, 4)  TD_PLAN(150, 5, 5, 6)  TD_PLAN(160, 10, 4, 4) TD_PLAN(180, 5, 6, 6)  TD_PLAN(192, 6, 8, 4)
 TD_PLAN(200, 5, 10, 4) TD_PLAN(216, 6, 6, 6)  TD_PLAN(240, 10, 6, 4) TD_PLAN(250, 5, 5, 10) TD_PLAN(256, 8, 8, 4)
 #undef TD_PLAN

@@ -2,12 +2,15 @@
 // configurations that fit the fast path; every other shape runs the general pass kernels (fft_steps.cuh).
 #include <type_traits>
 #include "fft_fused.cuh"
+#include "fft_cluster.cuh"
 
 namespace tddft {
 
 // (NY, NZ, threads per CTA, CTAs per SM the registers are budgeted for)
 #define TD_FOR_EACH_PLANE(X) X(72, 72, 216, 2) X(48, 48, 96, 5) X(24, 24, 96, 8) X(18, 20, 96, 8) X(96, 100, 360, 1) X(108, 108, 324, 1)
-#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12) X(96) X(108)
+#define TD_FOR_EACH_XLEN(X) X(72) X(48) X(24) X(12) X(96) X(108) X(128)
+// planes held by a cluster of two CTAs (fft_cluster.cuh): (NY, NZ, threads per CTA, CTAs per SM)
+#define TD_FOR_EACH_CPLANE(X) X(128, 128, 512, 1) X(96, 100, 256, 2) X(108, 108, 256, 2)
 
 // Launch policy, fixed after the round-1 measurements (profiles/r01g_summary.md, r01i_summary.md): persistent grids that walk
 // the units plane-major; L2 prefetch of the CTA's next work-grid plane (inverse kernels) but not of orbital planes (they are
@@ -64,6 +67,47 @@ static cudaError_t plane_dispatch(bool inverse, int lkind, int skind, const ZArg
     return cudaErrorInvalidValue;
 }
 
+template <int NY, int NZ, int NTHR, int MINB, bool INV, class Load, class Store>
+static cudaError_t cplane_launch(Load ld, Store st, const ZArgs& a, cudaStream_t s) {
+    static_assert(Two<NY>::ok && Two<NZ>::ok, "cluster plane kernel needs two-stage plans");
+    const size_t smem = sizeof(cplx) * (size_t)(NY / 2) * Two<NZ>::PITCH;
+    auto kern = plane_cluster_kernel<NY, NZ, NTHR, MINB, INV, Load, Store>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(NTHR); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 2;
+    static int resident[kMaxDevices] = {0};                   // clusters the device holds at once
+    const int dev = current_device();
+    if (!resident[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        int sms = 0; cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cfg.gridDim = dim3(2 * sms * MINB);
+        int ncl = 0;
+        e = cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg);
+        if (e != cudaSuccess || ncl < 1) { cudaGetLastError(); ncl = sms * MINB / 2; }
+        resident[dev] = ncl;
+    }
+    const int nx = (int)(a.npencils / NY), nunits = nx * a.batch;
+    cfg.gridDim = dim3(2 * (unsigned)(nunits < resident[dev] ? nunits : resident[dev]));
+    return cudaLaunchKernelEx(&cfg, kern, ld, st, nx, nunits, a.tw2, a.tw);
+}
+template <int NY, int NZ, int NTHR, int MINB>
+static cudaError_t cplane_dispatch(bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t s) {
+    LoadWorkC lw{a.work, a.wstride, a.cmap, a.ncols, a.whint};
+    StoreWorkC sw{a.work, a.wstride, a.cmap, a.ncols, a.whint};
+    const BatchLayout lay{a.chunked, a.fbase, a.ftotal * CHUNK, a.nr};
+    if (!inverse) {
+        if (lkind == ZL_PAIR) return cplane_launch<NY, NZ, NTHR, MINB, false>(LoadPair{a.phi, a.phi2 ? a.phi2 : a.phi, a.pairs, a.npairs, a.nr}, sw, a, s);
+        if (lkind == ZL_PACK2) return cplane_launch<NY, NZ, NTHR, MINB, false>(LoadPack2{a.src0, a.src1, a.nfun, lay, a.lscale}, sw, a, s);
+        return cudaErrorInvalidValue;
+    }
+    if (skind == ZS_SPLIT2) return cplane_launch<NY, NZ, NTHR, MINB, true>(lw, StoreSplit2{a.dst, a.nfun, lay, a.sscale, kStreamHint, a.slots}, a, s);
+    return cudaErrorInvalidValue;
+}
+
 template <int NX>
 static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     static_assert(Two<NX>::ok, "fused x pass needs a two-stage plan");
@@ -106,12 +150,20 @@ bool fused_supported(const int* n) {
 #undef X
 #define X(NY, NZ, T, B) if (n[1] == NY && n[2] == NZ) pl = true;
     TD_FOR_EACH_PLANE(X)
+    TD_FOR_EACH_CPLANE(X)
 #undef X
     return px && pl;
 }
 cudaError_t launch_plane(int ny, int nz, bool inverse, int lkind, int skind, const ZArgs& a, cudaStream_t st) {
+    // a.cluster: prefer the two-CTA cluster kernel where the shape has both (the only one for 128 x 128)
+#define X(NY, NZ, T, B) if (a.cluster && ny == NY && nz == NZ) return cplane_dispatch<NY, NZ, T, B>(inverse, lkind, skind, a, st);
+    TD_FOR_EACH_CPLANE(X)
+#undef X
 #define X(NY, NZ, T, B) if (ny == NY && nz == NZ) return plane_dispatch<NY, NZ, T, B>(inverse, lkind, skind, a, st);
     TD_FOR_EACH_PLANE(X)
+#undef X
+#define X(NY, NZ, T, B) if (ny == NY && nz == NZ) return cplane_dispatch<NY, NZ, T, B>(inverse, lkind, skind, a, st);
+    TD_FOR_EACH_CPLANE(X)
 #undef X
     return cudaErrorInvalidValue;
 }

@@ -462,7 +462,7 @@ template <int NX> struct XCfg {
     static constexpr int R1 = Two<NX>::R1, R2 = Two<NX>::R2;
     static constexpr int G = R1 > R2 ? R1 : R2;
     static constexpr int NTHR = G * XW;
-    static constexpr int MINB = G > 9 ? 2 : 3;          // CTAs per SM the registers are budgeted for (radix-12 butterflies need more)
+    static constexpr int MINB = G > 12 ? 1 : (G > 9 ? 2 : 3);   // CTAs per SM the registers are budgeted for (radix-12 / radix-16 butterflies need more)
     static constexpr size_t SMEM = sizeof(cplx) * NX * XW;
 };
 // Twiddles: the residue / block index g = tid / XW is the warp index (XW = 32), so every stage dispatches on g to a

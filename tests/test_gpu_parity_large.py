@@ -128,13 +128,17 @@ def test_apply_config3_sampled_columns(mode):
 ])
 def test_apply_large_fft_plans(grid, lattice, ecut, nocc, nvec):
     case = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid))      # oracle with its own radix FFT
-    general = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid), oracle=False, fft_path=1) if grid == (96, 96, 100) else None
+    general = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid), oracle=False, fft_path=1) if grid != (108, 108, 108) else None
+    cluster = Case(lattice, grid, ecut, 2, nocc, 0.3, seed=sum(grid), oracle=False, fft_path=2) if grid != (128, 128, 128) else None
     for mode in (0, 1):
         X = case.trial(nvec, mode)
         ref = case.oracle.apply(X, mode)
-        assert rel_fro(case.gpu_apply(X, mode), ref) < TOL                 # 96 x 96 x 100: the fused plane / x kernels (1 CTA per SM)
+        # default path: fused plane / x kernels (96 x 100 and 108 x 108: one CTA per SM; 128 x 128: a cluster of two CTAs per plane)
+        assert rel_fro(case.gpu_apply(X, mode), ref) < TOL
         if general is not None:
-            assert rel_fro(general.gpu_apply(X, mode), ref) < TOL          # and the general pass kernels on the same shape
+            assert rel_fro(general.gpu_apply(X, mode), ref) < TOL          # the general pass kernels on the same shape
+        if cluster is not None:
+            assert rel_fro(cluster.gpu_apply(X, mode), ref) < TOL          # the two-CTA cluster plane kernel where the shape has both
 
 
 def test_apply_config4_shape_with_block_at_a_time_plan():

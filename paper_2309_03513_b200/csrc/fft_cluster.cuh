@@ -51,19 +51,27 @@ __global__ void __launch_bounds__(NTHR, MINB) plane_cluster_kernel(Load ld, Stor
         const int xpl = u / nbatch, b = u - xpl * nbatch;
         BL L = bind(ld, b, xpl, (long)xpl * NY * NZ);
         const auto S = bind(st, b, xpl, (long)xpl * NY * NZ);
+        {   // operands of the unit this cluster takes next -> L2 (each CTA its half of the threads' share; no registers held)
+            const int un = u + ncl;
+            if (un < nunits) { const int xn = un / nbatch, bn = un - xn * nbatch; bind(ld, bn, xn, (long)xn * NY * NZ).prefetch_l2(NY * NZ, tid + (int)h * NTHR, 2 * NTHR); }
+        }
         if constexpr (!INV) {
             // z stage 1 on the own rows: global -> registers -> shared
-            for (int t = tid; t < HY * R2z; t += NTHR) {
-                const int yl = t / R2z, i = t - yl * R2z, y = (int)h * HY + yl;
-                cplx x[R1z];
+            auto z1 = [&](auto mode_) {
+                constexpr int MD = decltype(mode_)::value;
+                for (int t = tid; t < HY * R2z; t += NTHR) {
+                    const int yl = t / R2z, i = t - yl * R2z, y = (int)h * HY + yl;
+                    cplx x[R1z];
 #pragma unroll
-                for (int r = 0; r < R1z; ++r) { const Raw q = L.template fetch<0>(y * NZ + i + R2z * r); x[r] = L.make(q); }
-                Dft<R1z, false>::run(x);
-                cplx* row = sm + yl * PITCH;
-                row[TZ::pad(i)] = x[0];
+                    for (int r = 0; r < R1z; ++r) { const Raw q = L.template fetch<MD>(y * NZ + i + R2z * r); x[r] = L.make(q); }
+                    Dft<R1z, false>::run(x);
+                    cplx* row = sm + yl * PITCH;
+                    row[TZ::pad(i)] = x[0];
 #pragma unroll
-                for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], __ldg(twz_g + i * k));
-            }
+                    for (int k = 1; k < R1z; ++k) row[TZ::pad(i + R2z * k)] = cmul(x[k], __ldg(twz_g + i * k));
+                }
+            };
+            if (BL::kModes > 1 && L.mode() == 1) z1(IC<1>{}); else z1(IC<0>{});
             __syncthreads();
             for (int t = tid; t < HY * R1z; t += NTHR) {      // z stage 2, in place
                 const int yl = t / R1z, k1 = t - yl * R1z;

@@ -109,8 +109,34 @@ static cudaError_t cplane_dispatch(bool inverse, int lkind, int skind, const ZAr
 }
 
 template <int NX>
+static cudaError_t xpass_generic_launch(int mode, const SArgs& a, cudaStream_t s) {
+    constexpr size_t smem = XGCfg<NX>::SMEM;
+    static int resident_d[kMaxDevices] = {0};
+    const int dev = current_device();
+    if (!resident_d[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(xpass_generic_kernel<NX, SM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_generic_kernel<NX, SM_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(xpass_generic_kernel<NX, SM_CONV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        int sms = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, xpass_generic_kernel<NX, SM_CONV>, XGCfg<NX>::NTHR, smem);
+        resident_d[dev] = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    const unsigned tiles = (unsigned)((a.inner + XGCfg<NX>::XWG - 1) / XGCfg<NX>::XWG);
+    int gy = 1;      // at least 3 waves of the resident CTAs (or one grid per CTA)
+    while (gy < a.batch && (long)tiles * gy < 3L * resident_d[dev]) ++gy;
+    dim3 grid(tiles, (unsigned)gy);
+    constexpr int NT = XGCfg<NX>::NTHR;
+    if (mode == SM_FWD) return launch_pdl(xpass_generic_kernel<NX, SM_FWD>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    if (mode == SM_INV) return launch_pdl(xpass_generic_kernel<NX, SM_INV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    return launch_pdl(xpass_generic_kernel<NX, SM_CONV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+}
+template <int NX>
 static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     static_assert(Two<NX>::ok, "fused x pass needs a two-stage plan");
+    if constexpr (XCfg<NX>::G > 12) return xpass_generic_launch<NX>(mode, a, s);
+    else {
     constexpr size_t smem = XCfg<NX>::SMEM;
     static int resident_d[kMaxDevices] = {0};
     const int dev = current_device();
@@ -141,6 +167,7 @@ static cudaError_t xpass_launch(int mode, const SArgs& a, cudaStream_t s) {
     if (mode == SM_FWD) return launch_pdl(xpass_kernel<NX, SM_FWD>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
     if (mode == SM_INV) return launch_pdl(xpass_kernel<NX, SM_INV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
     return launch_pdl(xpass_kernel<NX, SM_CONV>, grid, NT, smem, s, a.work, a.inner, a.nr, a.batch, a.tw, a.ktab, a.whint);
+    }
 }
 
 bool fused_supported(const int* n) {

@@ -550,4 +550,86 @@ __global__ void __launch_bounds__(XCfg<NX>::NTHR, XCfg<NX>::MINB) xpass_kernel(c
     }
 }
 
+// ---- x pass, generic body (long lengths) ----------------------------------------------------------------------------
+// xpass_kernel gives every warp its own unrolled body with literal twiddles: 16 bodies for 128 = 16*8 are 6300 instructions (38 % of
+// its stall samples wait for instruction fetch) and only the 8 residue warps of 16 work in the radix-16 stages.  Here every thread
+// runs the same code over (butterfly, column) items, twiddles exp(-2 pi i g k / NX) from the table (L1 hits), XWG columns per CTA.
+template <int NX> struct XGCfg {
+    static constexpr int R1 = Two<NX>::R1, R2 = Two<NX>::R2;
+    static constexpr int XWG = 32, NTHR = 256;
+    static constexpr size_t SMEM = sizeof(cplx) * NX * XWG;
+};
+template <int NX, int MODE>
+__global__ void __launch_bounds__(XGCfg<NX>::NTHR, 2) xpass_generic_kernel(cplx* __restrict__ work, long inner, long nr, int batch,
+                                                                            const cplx* __restrict__ tw_g, const double* __restrict__ ktab, int hint) {
+    pdl_launch_dependents();
+    const unsigned long long pol = l2_policy(hint);
+    constexpr int R1 = XGCfg<NX>::R1, R2 = XGCfg<NX>::R2, XWG = XGCfg<NX>::XWG, NTHR = XGCfg<NX>::NTHR;
+    extern __shared__ cplx sm[];
+    const int tid = threadIdx.x;
+    pdl_wait();
+    for (int b = blockIdx.y; b < batch; b += gridDim.y) {
+        cplx* gbase = work + (long)b * nr + (long)blockIdx.x * XWG;
+        if (MODE == SM_FWD || MODE == SM_CONV) {
+            for (int t = tid; t < R2 * XWG; t += NTHR) {      // stage R1 forward of residue g: rows g + R2*r, twiddle after
+                const int g = t / XWG, c = t - g * XWG;
+                const bool live = (long)blockIdx.x * XWG + c < inner;
+                cplx x[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) x[r] = live ? ld_pol(gbase + (long)(g + R2 * r) * inner + c, pol) : make_double2(0.0, 0.0);
+                Dft<R1, false>::run(x);
+                sm[g * XWG + c] = x[0];
+#pragma unroll
+                for (int k = 1; k < R1; ++k) sm[(g + R2 * k) * XWG + c] = cmul(x[k], __ldg(tw_g + g * k));
+            }
+            __syncthreads();
+        }
+        for (int t = tid; t < R1 * XWG; t += NTHR) {          // block g: rows g*R2 + i
+            const int g = t / XWG, c = t - g * XWG;
+            const long col = (long)blockIdx.x * XWG + c;
+            const bool live = col < inner;
+            cplx x[R2];
+            if (MODE == SM_INV) {
+#pragma unroll
+                for (int i = 0; i < R2; ++i) x[i] = live ? ld_pol(gbase + (long)(g * R2 + i) * inner + c, pol) : make_double2(0.0, 0.0);
+            } else {
+#pragma unroll
+                for (int i = 0; i < R2; ++i) x[i] = sm[(g * R2 + i) * XWG + c];
+                Dft<R2, false>::run(x);
+            }
+            if (MODE == SM_FWD) {
+                if (live) {
+#pragma unroll
+                    for (int k = 0; k < R2; ++k) st_pol(gbase + (long)(g * R2 + k) * inner + c, x[k], pol);
+                }
+            } else {
+                if (MODE == SM_CONV) {
+#pragma unroll
+                    for (int k = 0; k < R2; ++k) { const double kt = live ? __ldg(ktab + (long)(g * R2 + k) * inner + col) : 0.0; x[k].x *= kt; x[k].y *= kt; }
+                }
+                Dft<R2, true>::run(x);
+#pragma unroll
+                for (int i = 0; i < R2; ++i) sm[(g * R2 + i) * XWG + c] = x[i];
+            }
+        }
+        if (MODE != SM_FWD) {
+            __syncthreads();
+            for (int t = tid; t < R2 * XWG; t += NTHR) {      // stage R1 inverse of residue g: conjugate twiddle, butterfly, natural order out
+                const int g = t / XWG, c = t - g * XWG;
+                const bool live = (long)blockIdx.x * XWG + c < inner;
+                cplx x[R1];
+                x[0] = sm[g * XWG + c];
+#pragma unroll
+                for (int k = 1; k < R1; ++k) x[k] = cmulc(sm[(g + R2 * k) * XWG + c], __ldg(tw_g + g * k));
+                Dft<R1, true>::run(x);
+                if (live) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) st_pol(gbase + (long)(g + R2 * r) * inner + c, x[r], pol);
+                }
+            }
+        }
+        __syncthreads();        // the tile is reused by the next grid of the batch
+    }
+}
+
 }  // namespace tddft

@@ -251,6 +251,7 @@ def main():
     ap.add_argument("--workspace-gb", type=float, default=0.0)
     ap.add_argument("--work-l2-mb", type=float, default=0.0)
     ap.add_argument("--tile-width", type=int, default=0)
+    ap.add_argument("--plan", type=int, default=0, help="0 auto, 1 resident, 2 streamed")
     ap.add_argument("--davidson", type=int, default=0, help="also run tddft_davidson for this many roots (not timed into `value`)")
     ap.add_argument("--max-iter", type=int, default=0)
     ap.add_argument("--precond", type=int, default=0)
@@ -289,7 +290,7 @@ def main():
     d_psi = [torch.from_numpy(p).cuda() for p in inp["psi"]]
     opts = {}
     for k, v in (("pair_tile", args.pair_tile), ("fft_batch", args.fft_batch), ("max_iter", args.max_iter), ("fft_path", args.fft_path),
-                 ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("tile_width", args.tile_width), ("precond", args.precond), ("verbose", args.verbose)):
+                 ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("tile_width", args.tile_width), ("plan", args.plan), ("precond", args.precond), ("verbose", args.verbose)):
         if v:
             opts[k] = v
     ctx = b.tddft_init(cfg["lattice"], cfg["grid"], cfg["ecut"], cfg["nspin"], cfg["nocc"], d_psi[0],

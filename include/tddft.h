@@ -105,6 +105,9 @@ typedef struct {
   double work_l2_mb;
   int tile_width;           /* most columns of an off-diagonal tile of the exchange loop (rounded down to a multiple of the tile edge);
                              * <= 0 = as wide as the workspace allows */
+  int plan;                 /* memory plan of tddft_apply_liouville: 0 = resident if it fits, else streamed (default); 1 = resident only
+                             * (TDDFT_ENOMEM if it does not fit); 2 = streamed (tile loop outermost, pair potentials formed once whatever nvec,
+                             * a(r) recomputed per tile, contributions added in the sphere) */
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,

@@ -37,7 +37,7 @@ class tddft_options(C.Structure):
         ("pair_list_up", C.c_void_p), ("n_pairs_up", C.c_long), ("pair_list_dn", C.c_void_p), ("n_pairs_dn", C.c_long),
         ("ace", C.c_int), ("psi_ace_up", C.c_void_p), ("n_ace_extra_up", C.c_int),
         ("psi_ace_dn", C.c_void_p), ("n_ace_extra_dn", C.c_int),
-        ("work_l2_mb", C.c_double), ("tile_width", C.c_int),
+        ("work_l2_mb", C.c_double), ("tile_width", C.c_int), ("plan", C.c_int),
     ]
 
 

@@ -387,11 +387,19 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
     };
     fixed = fixed_bytes();
     auto need = [&](int T_, int W_, int ks_) { return fixed + grid_b * ((size_t)T_ * W_ + 2 * (size_t)(T_ + W_) * ks_); };
-    for (;;) {
-        if (need(T, T, ks) <= budget) break;
-        if (ks > 1 && (ks > 8 || T <= 48)) { do { ++nks; } while ((nvec + nks - 1) / nks == ks); ks = (nvec + nks - 1) / nks; continue; }
-        if (T > 2) { T = std::max(2, T - (T > 16 ? 4 : 1)); continue; }
-        return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the streamed plan");
+    // all vectors together with a tile edge down to 3/4 of the preferred one, else fewer vectors at a time (tau is formed once either
+    // way; ks <= 8 runs the half-width DMMA tiles of the contraction), else ever smaller tiles
+    {
+        const int T0 = T;
+        bool found = false;
+        for (;;) {
+            const int tmin = ks == 1 ? std::min(T0, 2) : std::min(T0, std::max(48, 3 * T0 / 4));
+            for (T = T0; T >= tmin; T -= (T > 16 ? 4 : 1)) if (need(T, T, ks) <= budget) { found = true; break; }
+            if (found) break;
+            if (ks == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the streamed plan");
+            do { ++nks; } while ((nvec + nks - 1) / nks == ks);
+            ks = (nvec + nks - 1) / nks;
+        }
     }
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }
     int W = T;
@@ -475,6 +483,19 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
         else { StageTimer t(c, ST_S6); TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1; }
         const bool has_init = hxc || sfk || c->vloc[bl.tgt];
         const PairTiles& pt = c->tiles[bl.src];
+        // Row-resident mode (all trial vectors fit at once): the tiles of one row block follow each other (build_tiles), so a[I] is
+        // transformed once per row block and out[I] collects the whole row in real space before it goes back to the sphere; only
+        // the column side (a[J], out[J]) is per tile.  The batch layout is fixed: rows at functions [0, T*ks), columns from T*ks.
+        const bool row_mode = ks == nvec;
+        const long ftot_row = (long)(T + W) * ks;
+        int row_i0 = -1, row_ti = 0;
+        auto flush_row = [&]() -> int {      // S6 of the finished row block
+            if (row_i0 < 0) return TDDFT_OK;
+            StageTimer tm(c, ST_S6);
+            const FunLayout dI{dvlen, dboff + (long)row_i0 * npwh, npwh, ks, 0};
+            row_i0 = -1;
+            return to_sphere_plus_d(c, O_, row_ti * ks, nullptr, dst, dI, nullptr, 0, ftot_row, true);
+        };
         for (const TileInfo& t : pt.tiles) {
             const bool exch = c->alpha != 0.0 && t.npairs > 0;
             if (!exch && !(t.diag && has_init)) continue;
@@ -482,6 +503,35 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
                 StageTimer tm(c, ST_S4);
                 if (t.partial) TD_CUDA(c, cudaMemsetAsync(tau, 0, grid_b * (size_t)t.nslots, c->stream));
                 rc = pair_potentials_dev(c, phi, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1, t.nslots); if (rc) return rc;
+            }
+            if (row_mode) {
+                const int nI = t.ti * ks, nJ = t.diag ? 0 : t.tj * ks;
+                const long fJ = (long)T * ks;
+                if (t.i0 != row_i0) {          // a new row block: a[I], and out[I] = phi V + V_loc a (Eq. 4; zero if neither)
+                    TD_RC(flush_row());
+                    { StageTimer tm(c, ST_S1);
+                      TD_RC(to_real_space(c, src, FunLayout{vlen, boff + (long)t.i0 * npwh, npwh, ks, 0}, nI, A, 1, 0, ftot_row)); }
+                    StageTimer tm(c, ST_S5);
+                    TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] : nullptr, c->vloc[bl.tgt], A, t.ti, ks, nr, O_, c->stream, ftot_row));
+                    c->stats.kernel_launches += 1;
+                    row_i0 = t.i0; row_ti = t.ti;
+                }
+                if (nJ) {
+                    { StageTimer tm(c, ST_S1);
+                      TD_RC(to_real_space(c, src, FunLayout{vlen, boff + (long)t.j0 * npwh, npwh, ks, 0}, nJ, A, 1, fJ, ftot_row)); }
+                    StageTimer tm(c, ST_S5);      // zero the column part of every chunk of out
+                    TD_CUDA(c, cudaMemset2DAsync(O_ + fJ * CHUNK, sizeof(double) * ftot_row * CHUNK, 0, sizeof(double) * (size_t)nJ * CHUNK, (size_t)((nr + CHUNK - 1) / CHUNK), c->stream));
+                }
+                if (exch) {
+                    StageTimer tm(c, ST_S5);
+                    TD_CUDA(c, launch_contract_full(t.diag, O_, A, tau, 0, t.ti, t.diag ? 0 : T, t.tj, ks, ftot_row, t.nslots, nr, c->alpha, c->stream));
+                    c->stats.kernel_launches += (ks + 15) / 16;
+                }
+                if (nJ) {
+                    StageTimer tm(c, ST_S6);
+                    TD_RC(to_sphere_plus_d(c, O_, nJ, nullptr, dst, FunLayout{dvlen, dboff + (long)t.j0 * npwh, npwh, ks, 0}, nullptr, fJ, ftot_row, true));
+                }
+                continue;
             }
             for (int k0 = 0; k0 < nvec; k0 += ks) {
                 const int kcc = std::min(ks, nvec - k0);
@@ -504,6 +554,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
                 if (nJ) TD_RC(to_sphere_plus_d(c, O_, nJ, nullptr, dst, dJ, nullptr, nI, ftot, true));
             }
         }
+        TD_RC(flush_row());
         if (rotb) {       // Eq. 31: rotate the grid part back and add D
             StageTimer t(c, ST_S7X);
             TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1;
@@ -566,9 +617,12 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
         while (T > tmin && fixed + grid_b * (size_t)T * T > budget) T = std::max(tmin, T - 4);
         const bool fits = fixed + grid_b * (size_t)T * T <= budget;
         // a small tile costs a(r)/out(r) traffic in S5: before shrinking T below half its cap, give up residency of all blocks
-        if (fits && T >= std::min(maxsrc, tcap / 2)) break;
+        const int tfloor = c->pair_tile > 0 ? std::min(48, c->pair_tile) : 48;      // an explicitly small pair_tile is the caller's choice
+        if (c->plan == 2) { kc = 0; break; }
+        if (fits && T >= std::min(maxsrc, std::min(tcap / 2, c->pair_tile > 0 ? c->pair_tile : tcap))) break;
         if (resident && nblk > 1) { resident = false; continue; }
-        if (fits && T >= std::min(maxsrc, 48)) break;
+        if (fits && T >= std::min(maxsrc, tfloor)) break;
+        if (c->plan == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the resident plan");
         // a(r) / out(r) of a whole spin block do not fit for all trial vectors: tile loop outermost, tau formed once (apply_streamed)
         kc = 0;
         break;
@@ -771,6 +825,8 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->fused = opt->fft_path == 0 || opt->fft_path == 2;
             c->prefer_cluster = opt->fft_path == 2 ? 1 : 0;
             c->tile_width = opt->tile_width;
+            if (opt->plan < 0 || opt->plan > 2) return fail(TDDFT_EINVAL, "init: plan must be 0, 1 or 2");
+            c->plan = opt->plan;
             if (opt->work_l2_mb > 0) c->work_l2_mb = opt->work_l2_mb;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
             if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");

@@ -38,7 +38,7 @@ struct tddft_ctx {
     cudaStream_t stream = nullptr;
     double workspace_gb = 0;
     double work_l2_mb = 48.0;        // launches with smaller work grids keep them under the normal L2 policy
-    int pair_tile = 0, fft_batch = 0, tile_width = 0;
+    int pair_tile = 0, fft_batch = 0, tile_width = 0, plan = 0;
     int num_sms = 148;
     int prefer_cluster = 0;          // fft_path = 2: two-CTA cluster plane kernels where a shape has both variants
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off

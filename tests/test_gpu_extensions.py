@@ -212,7 +212,7 @@ def test_coupling_closed_shell_and_k_chunks():
 def test_streamed_plan_rotation_truncation_sf_kernel_and_ace():
     import torch
     from paper_2309_03513_b200 import binding as b
-    cap = dict(workspace_gb=0.0025, pair_tile=4)
+    cap = dict(plan=2, pair_tile=4)          # all vectors at once: the row-resident mode of the streamed plan
     rng = np.random.default_rng(16)
     U = [inputs.random_orthogonal(rng, 6), inputs.random_orthogonal(rng, 4)]
     mask = [_random_mask(rng, 6, 0.6), _random_mask(rng, 4, 0.6)]

@@ -104,19 +104,20 @@ def test_host_buffer_entry_point_equals_device_path(mode):
         assert np.array_equal(AXp.numpy(), ref)
 
 
+@pytest.mark.parametrize("cap", [dict(workspace_gb=0.002), dict(plan=2)])      # vectors in inner chunks / all vectors at once (row-resident mode)
 @pytest.mark.parametrize("mode", [0, 1, 2])
-def test_streamed_plan_forms_tau_once(mode):
+def test_streamed_plan_forms_tau_once(mode, cap):
     # A workspace cap under which a(r) / out(r) of a spin block do not fit for all trial vectors: the tile loop runs outermost
     # (api.cu: apply_streamed), tau is formed once whatever the number of vectors (Eq. 6), a(r) is recomputed per tile
     # and the tile contributions are added in the sphere.  Same operator: V_loc, Hxc, ragged tiles, vectors in inner chunks.
     from paper_2309_03513_b200 import binding as b
-    case = Case(TRI, (12, 18, 20), 6.0, 2, (9, 7), 0.3, seed=131, vloc=True, pair_tile=4, workspace_gb=0.003)
+    case = Case(TRI, (12, 18, 20), 6.0, 2, (9, 7), 0.3, seed=131, vloc=True, pair_tile=4, **cap)
     X = case.trial(5, mode)
     got = case.gpu_apply(X, mode)
     st = b.tddft_get_stats(case.ctx())
     n = [9, 7]
     unique = sum(k * (k + 1) // 2 for k in (n if mode == 0 else [n[mode - 1]]))
-    assert st["blocks_resident"] == 0 and st["pair_ffts"] == unique, st
+    assert st["blocks_resident"] == 0 and st["pair_ffts"] == unique and (st["k_chunk"] == 5) == ("plan" in cap), st
     assert rel_fro(got, case.oracle.apply(X, mode)) < TOL
 
 

@@ -174,8 +174,8 @@ typedef struct {
   int fft_path;  /* 0 = fused plane/x kernels, 1 = general pass kernels */
   int pair_batch; /* orbital pairs per launch of the pair-FFT pipeline in the last apply (<= 2*fft_batch) */
   int pair_tile;  /* tile edge of the last apply */
-  int k_chunk;    /* trial vectors processed together (< nvec: the pair potentials were recomputed per chunk) */
-  int blocks_resident; /* 1: the real-space functions of all spin blocks were resident; 0: one spin block at a time */
+  int k_chunk;    /* trial vectors processed together (< nvec only under the streamed plan: vectors looped inside a tile) */
+  int blocks_resident; /* 1: the real-space functions of all spin blocks were resident; 0: one spin block at a time, or the streamed plan */
   int tile_width;      /* columns of an off-diagonal tile of the last apply (a multiple of pair_tile) */
 } tddft_stats;
 int tddft_set_timing(tddft_ctx* ctx, int enabled); /* stage timing with CUDA events (adds synchronisation) */

@@ -387,13 +387,13 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
     };
     fixed = fixed_bytes();
     auto need = [&](int T_, int W_, int ks_) { return fixed + grid_b * ((size_t)T_ * W_ + 2 * (size_t)(T_ + W_) * ks_); };
-    // all vectors together with a tile edge down to 3/4 of the preferred one, else fewer vectors at a time (tau is formed once either
-    // way; ks <= 8 runs the half-width DMMA tiles of the contraction), else ever smaller tiles
+    // as many vectors together as a tile edge >= 48 allows (tau is formed once either way, but few vectors leave the DMMA tiles of the
+    // contraction mostly empty: measured at config 5, 8 vectors at tile 58: S5 15.8 s; 1 vector at tile 72: 98 s), else ever smaller tiles
     {
         const int T0 = T;
         bool found = false;
         for (;;) {
-            const int tmin = ks == 1 ? std::min(T0, 2) : std::min(T0, std::max(48, 3 * T0 / 4));
+            const int tmin = ks == 1 ? std::min(T0, 2) : std::min(T0, 48);
             for (T = T0; T >= tmin; T -= (T > 16 ? 4 : 1)) if (need(T, T, ks) <= budget) { found = true; break; }
             if (found) break;
             if (ks == 1) return set_err(c, TDDFT_ENOMEM, "workspace budget too small for the streamed plan");

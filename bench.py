@@ -252,6 +252,7 @@ def main():
     ap.add_argument("--work-l2-mb", type=float, default=0.0)
     ap.add_argument("--tile-width", type=int, default=0)
     ap.add_argument("--plan", type=int, default=0, help="0 auto, 1 resident, 2 streamed")
+    ap.add_argument("--shard-apply", action="store_true", help="N > 1: shard ONE block apply over the ranks (tiles dealt to the ranks, one all-reduce of AX; strong scaling) instead of one block per rank")
     ap.add_argument("--davidson", type=int, default=0, help="also run tddft_davidson for this many roots (not timed into `value`)")
     ap.add_argument("--max-iter", type=int, default=0)
     ap.add_argument("--precond", type=int, default=0)
@@ -283,12 +284,15 @@ def main():
     # ---- inputs: same orbitals on every rank, rank-specific trial-vector block (weak scaling over images) ----
     miller, g2 = b.tddft_enumerate_gvectors(cfg["lattice"], cfg["ecut"])
     inp = inputs.make_problem_inputs(cfg, g2, scale_nocc=cfg["nocc"])
-    rng = np.random.Generator(np.random.PCG64(cfg["seed"] + 1000 * (rank + 1)))
+    shard = args.shard_apply and world > 1
+    rng = np.random.Generator(np.random.PCG64(cfg["seed"] + 1000 * ((0 if shard else rank) + 1)))      # sharded: the same block on every rank
     inp["rng"] = rng
     nvec, mode = cfg["nvec"], args.mode
     Xh = inputs.make_trial_block(cfg, inp, nvec, mode)
     d_psi = [torch.from_numpy(p).cuda() for p in inp["psi"]]
     opts = {}
+    if shard:
+        opts["shard_rank"] = rank; opts["shard_count"] = world
     for k, v in (("pair_tile", args.pair_tile), ("fft_batch", args.fft_batch), ("max_iter", args.max_iter), ("fft_path", args.fft_path),
                  ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("tile_width", args.tile_width), ("plan", args.plan), ("precond", args.precond), ("verbose", args.verbose)):
         if v:
@@ -312,8 +316,9 @@ def main():
         return float(t.item())
 
     # ---- device-resident timing: K applies back to back, stage timing OFF (no host synchronisation inside) ----------
+    apply = (lambda: b.tddft_apply_liouville_sharded(ctx, dX, dAX, nvec, mode)) if shard else (lambda: b.tddft_apply_liouville(ctx, dX, dAX, nvec, mode))
     for _ in range(args.warmup):
-        b.tddft_apply_liouville(ctx, dX, dAX, nvec, mode)
+        apply()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -324,14 +329,14 @@ def main():
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
-        b.tddft_apply_liouville(ctx, dX, dAX, nvec, mode)
+        apply()
         st = b.tddft_get_stats(ctx)            # host counters only
         launches += st["kernel_launches"]; pair_ffts += st["pair_ffts"]
     e1.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     ms = max_over_ranks(e0.elapsed_time(e1))
-    value = world * nvec * args.steps / (ms * 1e-3)
+    value = (1 if shard else world) * nvec * args.steps / (ms * 1e-3)
 
     # ---- stage breakdown: a separate pass with CUDA events around every stage (adds a synchronisation per apply) -------
     b.tddft_set_timing(ctx, True)
@@ -348,7 +353,7 @@ def main():
 
     # ---- end to end through the C ABI with pinned host buffers ------------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not shard:
         Xp = torch.from_numpy(Xh).pin_memory()
         AXp = torch.empty_like(Xp).pin_memory()
         b.tddft_apply_liouville_host(ctx, Xp, AXp, nvec, mode)
@@ -374,7 +379,7 @@ def main():
         fp64 = {"dfma_tflops": dfma, "dmma_tflops": dmma}
         if args.probes:      # read bandwidth of the contraction's access pattern (32-byte pieces) against whole 256-byte runs
             fp64["read_gbs_by_piece_bytes"] = {str(pb_): b.tddft_stream_probe(ctx, pb_) for pb_ in (32, 64, 128, 256)}
-        if not args.no_coupling and mode == 0:
+        if not args.no_coupling and mode == 0 and not shard:
             b.tddft_apply_coupling(ctx, dX[:1], dAX[:1], 1, 0)      # warm-up
             torch.cuda.synchronize()
             e0.record(stream)
@@ -434,12 +439,12 @@ def main():
         cpu_baseline = oracle_sample(cfg)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": list(cfg["grid"]), "nocc": list(cfg["nocc"]), "nvec": nvec,
                    "mode": ["spin_conserving", "spin_flip_up_down", "spin_flip_down_up"][mode], "alpha": cfg["alpha"],
                    "pair_tile": st["pair_tile"], "tile_width": st["tile_width"], "k_chunk": st["k_chunk"], "blocks_resident": st["blocks_resident"],
-                   "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": "images x%d" % world},
+                   "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": ("one apply sharded over %d ranks (tiles dealt to the ranks, one all-reduce of AX)" if shard else "images x%d") % world},
         "block_applies_per_s": value / nvec,
         "pair_ffts_per_s": (world * pairs_per_step / (s4_ms * 1e-3)) if s4_ms > 0 else None,
         "pair_ffts_per_step": pairs_per_step,

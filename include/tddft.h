@@ -108,6 +108,13 @@ typedef struct {
   int plan;                 /* memory plan of tddft_apply_liouville: 0 = resident if it fits, else streamed (default); 1 = resident only
                              * (TDDFT_ENOMEM if it does not fit); 2 = streamed (tile loop outermost, pair potentials formed once whatever nvec,
                              * a(r) recomputed per tile, contributions added in the sphere) */
+  /* Sharding of ONE apply over several GPUs (the paper's band-group level).  With shard_count > 1 this
+   * context applies only the exchange tiles it owns (tiles are dealt to the shards by descending pair count) and only shard 0 adds
+   * the terms that are not sums over pairs (D, K1e, V_loc, ACE); every shard projects its partial result (P_c is linear).  The full
+   * A X is the SUM of the shards' outputs: one all-reduce of AX, done by the caller (binding.tddft_apply_liouville_sharded uses
+   * torch.distributed / NCCL).  Orbitals and X are replicated.  tddft_davidson must not be used with shard_count > 1. */
+  int shard_rank;
+  int shard_count;
 } tddft_options;
 
 /* Canonical half sphere (reading A7 of DESIGN.md): member iff |B^T m|^2 <= ecut_wfc_ry; half = G=0, then m1>0,

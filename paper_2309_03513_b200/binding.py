@@ -37,7 +37,7 @@ class tddft_options(C.Structure):
         ("pair_list_up", C.c_void_p), ("n_pairs_up", C.c_long), ("pair_list_dn", C.c_void_p), ("n_pairs_dn", C.c_long),
         ("ace", C.c_int), ("psi_ace_up", C.c_void_p), ("n_ace_extra_up", C.c_int),
         ("psi_ace_dn", C.c_void_p), ("n_ace_extra_dn", C.c_int),
-        ("work_l2_mb", C.c_double), ("tile_width", C.c_int), ("plan", C.c_int),
+        ("work_l2_mb", C.c_double), ("tile_width", C.c_int), ("plan", C.c_int), ("shard_rank", C.c_int), ("shard_count", C.c_int),
     ]
 
 
@@ -186,6 +186,23 @@ def tddft_workspace_bytes(ctx):
 def tddft_apply_liouville(ctx, X, AX, nvec, mode=TDDFT_SPIN_CONSERVING):
     """X, AX: CUDA torch tensors complex128 [nvec, vector_len] (AX is written)."""
     _check(_lib.tddft_apply_liouville(ctx._h, _ptr(X), _ptr(AX), C.c_int(nvec), C.c_int(mode)), ctx._h)
+
+
+def allreduce_sum_(t, group=None):
+    """Sum a tensor over the ranks of a torch.distributed group, in place (NCCL on CUDA tensors, gloo on CPU tensors)."""
+    import torch
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(torch.view_as_real(t) if t.is_complex() else t, op=dist.ReduceOp.SUM, group=group)
+    return t
+
+
+def tddft_apply_liouville_sharded(ctx, X, AX, nvec, mode, group=None):
+    """One apply sharded over the ranks of `group`: every rank holds a context created with shard_rank = its rank and
+    shard_count = the group size, the same orbitals and the same X; each applies the exchange tiles it owns and the partial results
+    are summed by ONE all-reduce of AX (NCCL over NVLink).  Argument marshalling + the collective only."""
+    tddft_apply_liouville(ctx, X, AX, nvec, mode)
+    return allreduce_sum_(AX, group)
 
 
 def tddft_apply_liouville_host(ctx, X_host, AX_host, nvec, mode=TDDFT_SPIN_CONSERVING):

@@ -322,6 +322,15 @@ int build_tiles(tddft_ctx* c, int spin, int T, int W) {
             pt.total_pairs += cnt;
             pt.tiles.push_back(t);
         }
+    // tiles dealt to the shards: heaviest first, each to the least loaded shard (the same list on every shard)
+    pt.owner.assign(pt.tiles.size(), 0);
+    if (c->shard_count > 1) {
+        std::vector<int> order(pt.tiles.size());
+        for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+        std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return pt.tiles[x].npairs > pt.tiles[y].npairs; });
+        std::vector<long> load(c->shard_count, 0);
+        for (int i : order) { const int r = (int)(std::min_element(load.begin(), load.end()) - load.begin()); pt.owner[i] = r; load[r] += pt.tiles[i].npairs; }
+    }
     const size_t np = std::max<size_t>(pairs.size(), 1);
     TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * np));
     TD_CUDA(c, cudaMalloc((void**)&pt.d_pslot, sizeof(int) * np));
@@ -367,6 +376,7 @@ struct Block { int src, tgt; long off; };   // occupied spin, target spin, offse
 static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const std::vector<Block>& blocks, bool hxc, bool sfk, long L, size_t budget) {
     const long nr = c->hp.nr, npwh = c->hp.npwh;
     const int nblk = (int)blocks.size();
+    const bool lead = c->shard_rank == 0;
     const size_t grid_b = sizeof(double) * (size_t)chunked_elems(1, nr);
     int maxsrc = 0, maxbasis = 0; bool rot = false;
     for (auto& b : blocks) {
@@ -479,9 +489,15 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
         cplx* dst = rotb ? Yr : AX;
         const long dvlen = rotb ? (long)no * npwh : L, dboff = rotb ? 0 : bl.off;
         FunLayout lay_full{L, bl.off, npwh, nvec, 0};
+        auto d_or_zero = [&]() -> int {      // AX block = D X on the lead shard, zero on the others
+            if (lead) { TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1; }
+            else TD_CUDA(c, cudaMemset2DAsync(AX + bl.off, sizeof(cplx) * L, 0, sizeof(cplx) * (size_t)no * npwh, nvec, c->stream));
+            return TDDFT_OK;
+        };
         if (rotb) TD_CUDA(c, cudaMemsetAsync(Yr, 0, sizeof(cplx) * (size_t)nvec * no * npwh, c->stream));
-        else { StageTimer t(c, ST_S6); TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1; }
-        const bool has_init = hxc || sfk || c->vloc[bl.tgt];
+        else { StageTimer t(c, ST_S6); TD_RC(d_or_zero()); }
+        const double* vloc_b = lead ? c->vloc[bl.tgt] : nullptr;
+        const bool has_init = hxc || sfk || vloc_b;
         const PairTiles& pt = c->tiles[bl.src];
         // Row-resident mode (all trial vectors fit at once): the tiles of one row block follow each other (build_tiles), so a[I] is
         // transformed once per row block and out[I] collects the whole row in real space before it goes back to the sphere; only
@@ -496,8 +512,9 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
             row_i0 = -1;
             return to_sphere_plus_d(c, O_, row_ti * ks, nullptr, dst, dI, nullptr, 0, ftot_row, true);
         };
-        for (const TileInfo& t : pt.tiles) {
-            const bool exch = c->alpha != 0.0 && t.npairs > 0;
+        for (size_t tidx = 0; tidx < pt.tiles.size(); ++tidx) {
+            const TileInfo& t = pt.tiles[tidx];
+            const bool exch = c->alpha != 0.0 && t.npairs > 0 && pt.owner[tidx] == c->shard_rank;
             if (!exch && !(t.diag && has_init)) continue;
             if (exch) {
                 StageTimer tm(c, ST_S4);
@@ -512,7 +529,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
                     { StageTimer tm(c, ST_S1);
                       TD_RC(to_real_space(c, src, FunLayout{vlen, boff + (long)t.i0 * npwh, npwh, ks, 0}, nI, A, 1, 0, ftot_row)); }
                     StageTimer tm(c, ST_S5);
-                    TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] : nullptr, c->vloc[bl.tgt], A, t.ti, ks, nr, O_, c->stream, ftot_row));
+                    TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] : nullptr, vloc_b, A, t.ti, ks, nr, O_, c->stream, ftot_row));
                     c->stats.kernel_launches += 1;
                     row_i0 = t.i0; row_ti = t.ti;
                 }
@@ -542,7 +559,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
                   TD_RC(to_real_space(c, src, layI, nI, A, 1, 0, ftot));
                   if (nJ) TD_RC(to_real_space(c, src, layJ, nJ, A, 1, nI, ftot)); }
                 { StageTimer tm(c, ST_S5);
-                  if (t.diag) { TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] + (long)k0 * nr : nullptr, c->vloc[bl.tgt], A, t.ti, kcc, nr, O_, c->stream, ftot)); c->stats.kernel_launches += 1; }
+                  if (t.diag) { TD_CUDA(c, launch_out_init(phi + (long)t.i0 * nr, (hxc || sfk) ? V[b] + (long)k0 * nr : nullptr, vloc_b, A, t.ti, kcc, nr, O_, c->stream, ftot)); c->stats.kernel_launches += 1; }
                   else TD_CUDA(c, cudaMemsetAsync(O_, 0, grid_b * (size_t)ftot, c->stream));
                   if (exch) {
                       TD_CUDA(c, launch_contract_full(t.diag, O_, A, tau, 0, t.ti, t.diag ? 0 : t.ti, t.tj, kcc, ftot, t.nslots, nr, c->alpha, c->stream));
@@ -557,10 +574,10 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
         TD_RC(flush_row());
         if (rotb) {       // Eq. 31: rotate the grid part back and add D
             StageTimer t(c, ST_S7X);
-            TD_CUDA(c, launch_d_term(X, AX, lay_full, no * nvec, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1;
+            TD_RC(d_or_zero());
             TD_RC(rotate_rows(c, bl.src, true, (const double*)Yr, 2L * no * npwh, (double*)(AX + bl.off), 2 * L, nvec, true));
         }
-        if (c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {
+        if (lead && c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {
             StageTimer t(c, ST_S7X);
             rc = lowrank_rows(c, (const double*)c->d_xi[bl.tgt], c->n_ace[bl.tgt], (const double*)(X + bl.off), (double*)(AX + bl.off), nvec * no, no, 2 * L,
                               -c->alpha, Oproj, o_cap);
@@ -588,8 +605,9 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     if (mode == TDDFT_SPIN_CONSERVING) { long off = 0; for (int s = 0; s < c->nspin; ++s) { blocks.push_back({s, s, off}); off += (long)c->nocc[s] * npwh; } }
     else { const int src = (mode == TDDFT_SPIN_FLIP) ? 0 : 1; blocks.push_back({src, 1 - src, 0}); }
     const int nblk = (int)blocks.size();
-    const bool hxc = (mode == TDDFT_SPIN_CONSERVING) && c->use_hartree_fxc;
-    const bool sfk = (mode != TDDFT_SPIN_CONSERVING) && c->sf_xc;        // K1e^SF of Eq. 24 with the kernel of Eq. 26
+    const bool lead = c->shard_rank == 0;      // sharded apply: only shard 0 adds the terms that are not sums over pairs
+    const bool hxc = lead && (mode == TDDFT_SPIN_CONSERVING) && c->use_hartree_fxc;
+    const bool sfk = lead && (mode != TDDFT_SPIN_CONSERVING) && c->sf_xc;        // K1e^SF of Eq. 24 with the kernel of Eq. 26
     int maxocc = 0, sumsrc = 0, maxsrc = 0, maxbasis = 0;
     bool rot = false;
     for (auto& b : blocks) {
@@ -709,12 +727,14 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
                 TD_CUDA(c, launch_scale_potential(c->d_fsf, drho[b], kcc, nr, V[b], c->stream)); c->stats.kernel_launches += 1;
             }
             { StageTimer t(c, ST_S5);
-              TD_CUDA(c, launch_out_init(phi, (hxc || sfk) ? V[b] : nullptr, c->vloc[bl.tgt], a[b], no, kcc, nr, out, c->stream)); c->stats.kernel_launches += 1; }
+              TD_CUDA(c, launch_out_init(phi, (hxc || sfk) ? V[b] : nullptr, lead ? c->vloc[bl.tgt] : nullptr, a[b], no, kcc, nr, out, c->stream)); c->stats.kernel_launches += 1; }
             // S4 + S5: exact-exchange response, tile by tile (Eq. 6; tau_vv' of PAPER.md:230)
             if (c->alpha != 0.0) {
                 const PairTiles& pt = c->tiles[bl.src];
-                for (const TileInfo& t : pt.tiles) {
+                for (size_t tidx = 0; tidx < pt.tiles.size(); ++tidx) {
+                    const TileInfo& t = pt.tiles[tidx];
                     if (t.npairs == 0) continue;            // every pair of the tile was truncated
+                    if (pt.owner[tidx] != c->shard_rank) continue;      // another shard's tile
                     { StageTimer tm(c, ST_S4);
                       if (t.partial) TD_CUDA(c, cudaMemsetAsync(tau, 0, grid_b * (size_t)t.nslots, c->stream));
                       rc = pair_potentials_dev(c, phi, phi, pt.d_pairs + t.pair_off, pt.d_pslot + t.pair_off, t.npairs, pt.batch_pairs, tau, 1, t.nslots); if (rc) return rc; }
@@ -729,12 +749,13 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
                 FunLayout layr{(long)no * npwh, 0, npwh, kcc, 0};
                 { StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, nullptr, Yr, layr, nullptr); if (rc) return rc; }
                 StageTimer t(c, ST_S7X);
-                TD_CUDA(c, launch_d_term(X, AX, lay, no * kcc, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1;
+                if (lead) { TD_CUDA(c, launch_d_term(X, AX, lay, no * kcc, c->d_kin, c->d_eig[bl.src], c->stream)); c->stats.kernel_launches += 1; }
+                else TD_CUDA(c, cudaMemset2DAsync(AX + (long)k0 * L + bl.off, sizeof(cplx) * L, 0, sizeof(cplx) * (size_t)no * npwh, kcc, c->stream));
                 TD_RC(rotate_rows(c, bl.src, true, (const double*)Yr, 2L * no * npwh, (double*)(AX + (long)k0 * L + bl.off), 2 * L, kcc, true));
             } else {
-                StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, X, AX, lay, c->d_eig[bl.src]); if (rc) return rc;
+                StageTimer t(c, ST_S6); rc = to_sphere_plus_d(c, out, no * kcc, lead ? X : nullptr, AX, lay, c->d_eig[bl.src]); if (rc) return rc;
             }
-            if (c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {   // H includes alpha V_X^ACE (Eqs. 28-30)
+            if (lead && c->n_ace[bl.tgt] > 0 && c->alpha != 0.0) {   // H includes alpha V_X^ACE (Eqs. 28-30)
                 StageTimer t(c, ST_S7X);
                 rc = lowrank_rows(c, (const double*)c->d_xi[bl.tgt], c->n_ace[bl.tgt], (const double*)(X + (long)k0 * L + bl.off),
                                   (double*)(AX + (long)k0 * L + bl.off), kcc * no, no, 2 * L, -c->alpha, O, o_cap);
@@ -827,6 +848,10 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
             c->tile_width = opt->tile_width;
             if (opt->plan < 0 || opt->plan > 2) return fail(TDDFT_EINVAL, "init: plan must be 0, 1 or 2");
             c->plan = opt->plan;
+            if (opt->shard_count > 1) {
+                if (opt->shard_rank < 0 || opt->shard_rank >= opt->shard_count) return fail(TDDFT_EINVAL, "init: shard_rank out of range");
+                c->shard_rank = opt->shard_rank; c->shard_count = opt->shard_count;
+            }
             if (opt->work_l2_mb > 0) c->work_l2_mb = opt->work_l2_mb;
             c->sf_xc = opt->sf_xc_kernel ? 1 : 0; if (opt->sf_cut > 0) c->sf_cut = opt->sf_cut;
             if (c->sf_xc && nspin != 2) return fail(TDDFT_EINVAL, "init: sf_xc_kernel needs nspin = 2");

@@ -16,6 +16,7 @@ struct TileInfo {
 struct PairTiles {
     int T = 0, W = 0, nocc = 0;
     std::vector<TileInfo> tiles;
+    std::vector<int> owner;    // shard that applies each tile (all 0 without sharding)
     int2* d_pairs = nullptr;   // pairs in processing order (sub-blocks of sbi x sbj, so a batch touches few orbitals)
     int* d_pslot = nullptr;    // tau slot of each pair of d_pairs
     int sbi = 0, sbj = 0, batch_pairs = 0;
@@ -39,6 +40,7 @@ struct tddft_ctx {
     double workspace_gb = 0;
     double work_l2_mb = 48.0;        // launches with smaller work grids keep them under the normal L2 policy
     int pair_tile = 0, fft_batch = 0, tile_width = 0, plan = 0;
+    int shard_rank = 0, shard_count = 1;   // sharding of one apply over GPUs: this context owns the tiles with owner == shard_rank
     int num_sms = 148;
     int prefer_cluster = 0;          // fft_path = 2: two-CTA cluster plane kernels where a shape has both variants
     bool fused = false;              // the grid shape has fused plane/x kernels (fft_fused.cu) and they are not switched off

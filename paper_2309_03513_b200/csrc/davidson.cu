@@ -229,6 +229,7 @@ int tddft_davidson(tddft_ctx* c, int nroots, int mode, double* evals, double* ev
     if (!evals || nroots < 1 || mode < 0 || mode > 2) return set_err(c, TDDFT_EINVAL, "davidson: bad argument");
     const long L = vector_len(c, mode);
     if (L < 0) return set_err(c, TDDFT_EINVAL, "spin flip needs nspin = 2");
+    if (c->shard_count > 1) return set_err(c, TDDFT_EINVAL, "davidson: not available on a sharded context (its applies would be partial sums)");
     TD_CUDA(c, cudaSetDevice(c->device));
     const long n2 = 2 * L, npwh = c->hp.npwh;
     cudaStream_t st = c->stream;

@@ -135,3 +135,25 @@ print("ok", rank)
                         "--master-addr", "127.0.0.1", "--master-port", "29617", str(script)],
                        capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stdout + r.stderr
+
+
+def test_sharded_apply_collective_two_ranks_gloo(tmp_path):
+    """The one exchange step of the sharded apply (binding.allreduce_sum_, used by tddft_apply_liouville_sharded): with gloo on CPU
+    tensors and world size 2 the partial results are summed on every rank, complex tensors through their real view."""
+    import subprocess, sys, textwrap
+    script = tmp_path / "w.py"
+    script.write_text(textwrap.dedent("""
+        import os, sys, torch, torch.distributed as dist
+        sys.path.insert(0, %r)
+        from paper_2309_03513_b200 import binding as b
+        dist.init_process_group("gloo")
+        r = dist.get_rank()
+        t = torch.full((3, 5), complex(r + 1.0, -(r + 1.0)), dtype=torch.complex128)
+        b.allreduce_sum_(t)
+        assert torch.allclose(t, torch.full((3, 5), complex(3.0, -3.0), dtype=torch.complex128)), t
+        dist.destroy_process_group()
+    """ % str(ROOT)))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29613")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+                        "--master-port", "29613", str(script)], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr

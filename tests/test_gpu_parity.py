@@ -125,3 +125,22 @@ def test_streamed_plan_closed_shell_and_no_exchange():
     case = Case(TRI, (12, 10, 9), 6.0, 1, (6,), 0.0, seed=132, workspace_gb=0.0004)
     X = case.trial(4, 0)
     assert rel_fro(case.gpu_apply(X, 0), case.oracle.apply(X, 0)) < TOL
+
+
+@pytest.mark.parametrize("plan", [1, 2])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_sharded_apply_partial_results_sum_to_the_full_operator(mode, plan):
+    # one apply sharded over GPUs.  Each shard applies the exchange tiles it owns, shard 0 adds D, K1e and V_loc, every
+    # shard projects its part; the sum over shards (one all-reduce of AX in tddft_apply_liouville_sharded) is A X.  Here the three
+    # shards run one after the other on the same GPU and the sum is taken on the host: the partition logic, without the collective.
+    full = Case(TRI, (12, 18, 20), 6.0, 2, (9, 7), 0.3, seed=141, vloc=True, pair_tile=4, plan=plan)
+    X = full.trial(3, mode)
+    ref = full.oracle.apply(X, mode)
+    total = np.zeros_like(ref)
+    for r in range(3):
+        shard = Case(TRI, (12, 18, 20), 6.0, 2, (9, 7), 0.3, seed=141, vloc=True, oracle=False, pair_tile=4, plan=plan, shard_rank=r, shard_count=3)
+        part = shard.gpu_apply(X, mode)
+        assert np.linalg.norm(part) > 0
+        total += part
+    assert rel_fro(total, ref) < TOL
+    assert rel_fro(full.gpu_apply(X, mode), ref) < TOL

@@ -252,6 +252,7 @@ def main():
     ap.add_argument("--work-l2-mb", type=float, default=0.0)
     ap.add_argument("--tile-width", type=int, default=0)
     ap.add_argument("--plan", type=int, default=0, help="0 auto, 1 resident, 2 streamed")
+    ap.add_argument("--emulate-shard", type=int, nargs=2, default=None, metavar=("RANK", "COUNT"), help="N = 1 only: time ONE shard of a sharded apply (partial result; a timing probe for the scaling estimate in DESIGN.md, not a bench value)")
     ap.add_argument("--shard-apply", action="store_true", help="N > 1: shard ONE block apply over the ranks (tiles dealt to the ranks, one all-reduce of AX; strong scaling) instead of one block per rank")
     ap.add_argument("--davidson", type=int, default=0, help="also run tddft_davidson for this many roots (not timed into `value`)")
     ap.add_argument("--max-iter", type=int, default=0)
@@ -293,6 +294,8 @@ def main():
     opts = {}
     if shard:
         opts["shard_rank"] = rank; opts["shard_count"] = world
+    elif args.emulate_shard and world == 1:
+        opts["shard_rank"], opts["shard_count"] = args.emulate_shard
     for k, v in (("pair_tile", args.pair_tile), ("fft_batch", args.fft_batch), ("max_iter", args.max_iter), ("fft_path", args.fft_path),
                  ("workspace_gb", args.workspace_gb), ("work_l2_mb", args.work_l2_mb), ("tile_width", args.tile_width), ("plan", args.plan), ("precond", args.precond), ("verbose", args.verbose)):
         if v:
@@ -444,7 +447,8 @@ def main():
         "config": {"workload": cfg["name"], "grid": list(cfg["grid"]), "nocc": list(cfg["nocc"]), "nvec": nvec,
                    "mode": ["spin_conserving", "spin_flip_up_down", "spin_flip_down_up"][mode], "alpha": cfg["alpha"],
                    "pair_tile": st["pair_tile"], "tile_width": st["tile_width"], "k_chunk": st["k_chunk"], "blocks_resident": st["blocks_resident"],
-                   "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": ("one apply sharded over %d ranks (tiles dealt to the ranks, one all-reduce of AX)" if shard else "images x%d") % world},
+                   "l2": "inputs_exceed_l2 (X, Phi(r), a(r), out(r), tau tiles >> 126 MB)", "parallelism": ("one apply sharded over %d ranks (tiles dealt to the ranks, one all-reduce of AX)" if shard else "images x%d") % world,
+                   **({"emulated_shard": list(args.emulate_shard)} if args.emulate_shard else {})},
         "block_applies_per_s": value / nvec,
         "pair_ffts_per_s": (world * pairs_per_step / (s4_ms * 1e-3)) if s4_ms > 0 else None,
         "pair_ffts_per_step": pairs_per_step,

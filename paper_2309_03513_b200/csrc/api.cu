@@ -322,15 +322,7 @@ int build_tiles(tddft_ctx* c, int spin, int T, int W) {
             pt.total_pairs += cnt;
             pt.tiles.push_back(t);
         }
-    // tiles dealt to the shards: heaviest first, each to the least loaded shard (the same list on every shard)
     pt.owner.assign(pt.tiles.size(), 0);
-    if (c->shard_count > 1) {
-        std::vector<int> order(pt.tiles.size());
-        for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
-        std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return pt.tiles[x].npairs > pt.tiles[y].npairs; });
-        std::vector<long> load(c->shard_count, 0);
-        for (int i : order) { const int r = (int)(std::min_element(load.begin(), load.end()) - load.begin()); pt.owner[i] = r; load[r] += pt.tiles[i].npairs; }
-    }
     const size_t np = std::max<size_t>(pairs.size(), 1);
     TD_CUDA(c, cudaMalloc((void**)&pt.d_pairs, sizeof(int2) * np));
     TD_CUDA(c, cudaMalloc((void**)&pt.d_pslot, sizeof(int) * np));
@@ -338,6 +330,21 @@ int build_tiles(tddft_ctx* c, int spin, int T, int W) {
     TD_CUDA(c, cudaMemcpyAsync(pt.d_pairs, pairs.data(), sizeof(int2) * pairs.size(), cudaMemcpyHostToDevice, c->stream));
     TD_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors go out of scope
     return TDDFT_OK;
+}
+
+// Sharded apply: the tiles of all spin blocks of the apply are dealt to the shards, heaviest first, each to the least loaded
+// shard (the same deterministic list on every shard).
+void assign_tile_owners(tddft_ctx* c, const std::vector<int>& spins) {
+    if (c->shard_count <= 1) return;
+    struct Item { int spin; int idx; long w; };
+    std::vector<Item> items;
+    for (int sp : spins) { PairTiles& pt = c->tiles[sp]; for (size_t i = 0; i < pt.tiles.size(); ++i) items.push_back({sp, (int)i, (long)pt.tiles[i].npairs}); }
+    std::stable_sort(items.begin(), items.end(), [](const Item& x, const Item& y) { return x.w > y.w; });
+    std::vector<long> load(c->shard_count, 0);
+    for (const Item& it : items) {
+        const int r = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+        c->tiles[it.spin].owner[it.idx] = r; load[r] += it.w;
+    }
 }
 
 size_t workspace_budget(const tddft_ctx* c) {
@@ -413,7 +420,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
     }
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }
     int W = T;
-    while (W < maxsrc - T && need(T, W + T, ks) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;
+    while (c->shard_count <= 1 && W < maxsrc - T && need(T, W + T, ks) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;
     int rc = ensure_arena(c, need(T, W, ks));
     if (rc) return rc;
     char* p = c->arena;
@@ -430,6 +437,7 @@ static int apply_streamed(tddft_ctx* c, const cplx* X, cplx* AX, int nvec, const
     double* Oproj = carve(sizeof(double) * o_cap);
     double* tau = carve(grid_b * (size_t)T * W);
     for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src]), W); if (rc) return rc; }
+    { std::vector<int> spins; for (auto& b : blocks) spins.push_back(b.src); assign_tile_owners(c, spins); }
     c->last_pair_tile = T; c->last_tile_width = W; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = ks; c->last_resident = 0;
 
     if (c->overlap_copies) for (int b = 0; b < nblk; ++b) TD_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_x_ready[b], 0));
@@ -650,7 +658,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     { const int nbk = (maxsrc + T - 1) / T; T = (maxsrc + nbk - 1) / nbk; }   // equal blocks: the kernel's cost follows the largest
     // width of the off-diagonal tiles: as many row blocks as the budget holds (at most what is right of the first row block)
     int W = T;
-    while (W < maxsrc - T && fixed + grid_b * (size_t)T * (W + T) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;
+    while (c->shard_count <= 1 && W < maxsrc - T && fixed + grid_b * (size_t)T * (W + T) <= budget && (c->tile_width <= 0 || W + T <= c->tile_width)) W += T;      // sharded: square tiles, more of them to deal out
     int rc = ensure_arena(c, fixed + grid_b * (size_t)T * W);
     if (rc) return rc;
     char* p = c->arena;
@@ -669,6 +677,7 @@ int apply_liouville_dev(tddft_ctx* c, const double* Xd, double* AXd, int nvec, i
     double* O = carve(sizeof(double) * o_cap);
     double* tau = carve(grid_b * (size_t)T * W);
     for (auto& b : blocks) { rc = build_tiles(c, b.src, std::min(T, c->nocc[b.src]), W); if (rc) return rc; }
+    { std::vector<int> spins; for (auto& b : blocks) spins.push_back(b.src); assign_tile_owners(c, spins); }
     c->last_pair_tile = T; c->last_tile_width = W; c->last_pair_batch = c->tiles[blocks[0].src].batch_pairs; c->last_kc = kc; c->last_resident = resident ? 1 : 0;
 
     for (int k0 = 0; k0 < nvec; k0 += kc) {

@@ -91,7 +91,7 @@ class ClockSampler:
 
 def ncu_traffic(pair_batch, workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of the S4 kernels per launch triple, from the tracked ncu summary
-    profiles/s4_traffic.csv (written from an `ncu --set full` capture, command in profiles/s4_traffic.md).  None when the
+    profiles/s4_traffic.csv (written from an `ncu --set full` capture, command in profiles/r02_summary.md).  None when the
     capture was taken with another pair batch or workload than the one running now."""
     path = os.path.join(ROOT, "profiles", "s4_traffic.csv")
     if not os.path.exists(path):

@@ -873,9 +873,10 @@ int tddft_init(tddft_ctx** out, const double* lattice, const int* grid, double e
         const long nr = c->hp.nr, npwh = c->hp.npwh;
         if (c->fft_batch <= 0) {
             // large launches win (measured up to 192 grids): with the plane-major unit order the CTAs of a launch share orbital
-            // planes whatever its size, and launch tails shrink; up to 96 grids and 640 MB of work grids, among the upper
-            // quarter the size whose plane units (n1 per grid) fill whole waves of two CTAs per SM best
-            const long cap = std::max<long>(1, std::min<long>(96, (640L << 20) / (16 * nr)));
+            // planes whatever its size, and launch tails shrink (S4 of NV215-72: 642 / 629 / 628 / 622 / 622 ms at 64 / 90 / 128 /
+            // 160 / 192 grids); up to 192 grids and 1.5 GB of work grids, among the upper quarter the size whose plane units
+            // (n1 per grid) fill whole waves of two CTAs per SM best
+            const long cap = std::max<long>(1, std::min<long>(192, (1536L << 20) / (16 * nr)));
             const long resident = 2L * c->num_sms;
             long bestb = cap; double beste = 0.0;
             for (long b = cap; b >= std::max<long>(1, cap - cap / 4); --b) {

@@ -197,6 +197,19 @@ int tddft_get_stats(const tddft_ctx* ctx, tddft_stats* out);
 int tddft_pair_potentials(tddft_ctx* ctx, int spin, const int* pairs, long n_pairs, double* tau);
 int tddft_project(tddft_ctx* ctx, int spin, double* Y, long nfun);
 int tddft_gram(tddft_ctx* ctx, const double* V, const double* W, int m, long n_complex, double* G);
+/* tddft_gram_static: the same Gram matrix for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Calls no cudaMalloc / cudaFree / allocating library routine and does not
+ * synchronise: the split-k partial sums, which tddft_gram keeps in the context's growable arena, go to a 4 MiB file-scope
+ * `static __device__` array that every GPU loading the library holds until exit (gram_static.cu).
+ *   V, W: DEVICE complex128 [m][n_complex] as for tddft_gram; G: DEVICE double [m][m], row-major, owned by the caller, valid
+ *   once the context's stream has passed the call.  m <= TDDFT_GRAM_STATIC_MAX_M, else TDDFT_EINVAL with a message naming the
+ *   limit; the number of k splits shrinks with m so that m * m * splits doubles fit (m <= 22: the splits of tddft_gram, bit-equal
+ *   result; larger m: another summation order, equal to rounding).
+ *   The array is shared by every context and stream of a device and keeps the last call's partial sums; each call overwrites all
+ *   it reads, so nothing is cleared, but two calls that overlap on the GPU (different streams) race on it: keep them ordered.
+ *   The first call on a device resolves the array's device address (cudaGetSymbolAddress): make it before a graph capture. */
+#define TDDFT_GRAM_STATIC_MAX_M 256
+int tddft_gram_static(tddft_ctx* ctx, const double* V, const double* W, int m, long n_complex, double* G);
 /* real-space orbital phi_v of a spin on the FFT grid, DEVICE double [n1*n2*n3] out */
 int tddft_orbital_real_space(tddft_ctx* ctx, int spin, int v, double* out);
 /* Overlap function S_mn of Eq. 32 between the orbitals the exchange term runs on (rotated by

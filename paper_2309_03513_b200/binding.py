@@ -20,7 +20,7 @@ EXPORTS = [
     "tddft_workspace_bytes", "tddft_apply_liouville", "tddft_apply_liouville_host", "tddft_davidson",
     "tddft_set_timing", "tddft_get_stats", "tddft_pair_potentials", "tddft_project", "tddft_gram",
     "tddft_orbital_real_space", "tddft_last_error", "tddft_destroy", "tddft_apply_coupling", "tddft_orbital_overlap",
-    "tddft_exchange_apply", "tddft_fp64_peak", "tddft_stream_probe",
+    "tddft_exchange_apply", "tddft_fp64_peak", "tddft_stream_probe", "tddft_gram_static",
 ]
 
 
@@ -247,6 +247,15 @@ def tddft_gram(ctx, V, W, m, n_complex):
     G = np.zeros((m, m), dtype=np.float64)
     _check(_lib.tddft_gram(ctx._h, _ptr(V), _ptr(W), C.c_int(m), C.c_long(n_complex), G.ctypes.data_as(C.c_void_p)), ctx._h)
     return G
+
+
+TDDFT_GRAM_STATIC_MAX_M = 256
+
+
+def tddft_gram_static(ctx, V, W, m, n_complex, G):
+    """G (DEVICE float64 [m][m]) = <V_i|W_j> with the partial sums in the library's static device array: no allocation, no
+    synchronisation; G is valid once the context's stream has passed the call (include/tddft.h)."""
+    _check(_lib.tddft_gram_static(ctx._h, _ptr(V), _ptr(W), C.c_int(m), C.c_long(n_complex), _ptr(G)), ctx._h)
 
 
 def tddft_orbital_real_space(ctx, spin, v, out):

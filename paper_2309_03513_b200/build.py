@@ -20,7 +20,7 @@ NGROUPS = 8
 
 def _units():
     units = []
-    for name in ("api.cu", "extensions.cu", "davidson.cu", "kernels.cu", "contract.cu", "gemm.cu", "fft_dispatch.cu", "fft_fused.cu"):
+    for name in ("api.cu", "extensions.cu", "davidson.cu", "kernels.cu", "contract.cu", "gemm.cu", "gram_static.cu", "fft_dispatch.cu", "fft_fused.cu"):
         units.append((os.path.join(CSRC, name), os.path.join(OBJ, name[:-3] + ".o"), []))
     units.append((os.path.join(CSRC, "plan.cpp"), os.path.join(OBJ, "plan.o"), ["-x", "cu"]))
     for g in range(NGROUPS):

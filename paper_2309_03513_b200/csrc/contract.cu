@@ -25,7 +25,9 @@
 // The partial sums of direction 2 (two row halves) meet in shared memory (double buffered) and are subtracted from out[J] one
 // stage later, behind the DMMAs of the next stage, in full 32-byte rows; the out[J] rows themselves are prefetched by cp.async two
 // iterations ahead.  out[I] leaves through shared memory at the end.  Diagonal tiles (DIAG) read the packed upper triangle
-// symmetrically and run direction 1 only.  No floating-point atomics: the summation order is fixed (reading A14).
+// symmetrically and run direction 1 only: without the B fragments of a[I] (168 registers) and without the partial-sum and out[J]
+// buffers (two stages = 64 KB) THREE of their CTAs fit an SM, three warps per scheduler instead of two.  No floating-point atomics:
+// the summation order is fixed (reading A14).
 //
 // What bounds it (measured, profiles/r02_summary.md): with the DMMAs removed the kernel takes 0.78 of its time, with the stage
 // copies removed 0.74: the CTA reads 32-byte pieces at a 256-byte stride (5.2 TB/s at best on this part, 7.4 TB/s for whole lines),
@@ -75,18 +77,19 @@ template <int NK, int MT> struct PipeCfg {
     static constexpr int STAGE_B = (TROWS + AROWS) * 32;    // bytes
     static constexpr int FL_B = AROWS * 32;                 // one buffer of direction-2 partial sums (one row half) / of out[J] rows
     static constexpr size_t SMEM = (size_t)NST * STAGE_B + 4 * FL_B + 3 * FL_B;
+    static constexpr size_t SMEM_DIAG = (size_t)2 * STAGE_B;        // diagonal tiles run direction 1 only: no partial-sum / out[J] buffers, two stages, three CTAs per SM
     static_assert(CHUNK % CP_P == 0 && IR % 8 == 6 && 2 * HALF >= IR, "fragment bank pattern / row coverage");
-    static_assert(2 * HALF * KB * 32 <= NST * STAGE_B, "prologue / epilogue stage the row block through the stage buffers");
+    static_assert(2 * HALF * KB * 32 <= 2 * STAGE_B, "prologue / epilogue stage the row block through the stage buffers");
 };
 __device__ __forceinline__ unsigned swz(int row, int piece) { return (unsigned)(row * 32 + ((piece ^ ((row >> 2) & 1)) << 4)); }
 
 template <int NK, bool DIAG, int MT>
-__global__ void __launch_bounds__(CP_NTHR, 2)
+__global__ void __launch_bounds__(CP_NTHR, DIAG ? 3 : 2)
 contract_pipe_kernel(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ tau,
                      int i0, int ti, int j0, int tj, int kc, int kn, long ftot, long stot, double alpha) {
     extern __shared__ __align__(128) char smc[];
     using C = PipeCfg<NK, MT>;
-    constexpr int KB = C::KB, IR = C::IR, JS = CP_JS, NST = C::NST, HALF = C::HALF;
+    constexpr int KB = C::KB, IR = C::IR, JS = CP_JS, NST = DIAG ? 2 : C::NST, HALF = C::HALF;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, lr = lane >> 2, lc = lane & 3;
     const int pp = w & 1, rh = w >> 1;
     const long chunk = blockIdx.x / (CHUNK / CP_P);
@@ -293,7 +296,7 @@ contract_pipe_kernel(double* __restrict__ out, const double* __restrict__ a, con
 template <int NK, bool DIAG, int MT>
 cudaError_t pipe_launch(long nchunks, double* out, const double* a, const double* tau, int i0, int ti, int j0, int tj,
                         int kc, int kn, long ftot, long stot, double alpha, cudaStream_t st) {
-    constexpr size_t smem = PipeCfg<NK, MT>::SMEM;
+    constexpr size_t smem = DIAG ? PipeCfg<NK, MT>::SMEM_DIAG : PipeCfg<NK, MT>::SMEM;
     static bool attr_done[kMaxDevices] = {false};
     const int dev = current_device();
     if (!attr_done[dev]) {
